@@ -1,0 +1,237 @@
+"""Seeded synthetic inputs for the Chebyshev-filter hot path (shared by oracle and CUDA path).
+
+This module holds NONE of the method's arithmetic: no GLL nodes, no mass matrix, no
+Hamiltonian, no recurrence.  It only fabricates the *inputs* the four C-ABI calls take
+(vectors, local fields sampled at caller-supplied node coordinates, atom positions,
+projector tables, SOC coupling matrices), from numpy `default_rng` streams, so that the
+CPU oracle (`oracle/`) and the CUDA library receive bit-identical arrays.
+
+The five workloads are BASELINE.json `configs[0..4]`; the readings of what the config
+sentences leave open are SURVEY.md §8(c) A13-A16 and are restated in DESIGN.md §4.
+The paper's own workloads (Table I: Fe3GeTe2 / twisted MoSe2 with SG15
+ONCV pseudopotentials on adaptive p=7 meshes) are not available; these inputs stand in
+for their shape only.
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+
+import numpy as np
+
+
+@dataclasses.dataclass(frozen=True)
+class Config:
+    """One BASELINE.json workload.  `ncell` cells per direction on a cube of side `L` Bohr."""
+    name: str
+    ncell: int
+    L: float
+    p: int
+    kfrac: tuple
+    nvec: int
+    chunk: int            # N_b: vectors per filter chunk (0 = all at once)
+    natoms: int
+    nproj: int            # projectors per atom (4: one radial x {s,px,py,pz}; 8: two radials)
+    degree: int           # Chebyshev degree m (paper's q)
+    prec: str             # "fp64" | "fp32" (H.X product precision inside eq. 11)
+    ngauss: int = 0       # >0: that many seeded Gaussian wells (config 0); 0: one per atom
+
+    @property
+    def n1(self) -> int:
+        return self.ncell * self.p
+
+    @property
+    def nnodes(self) -> int:
+        return self.n1 ** 3
+
+
+CONFIGS = {
+    0: Config("c0", 4, 8.0, 4, (0.0, 0.0, 0.0), 16, 0, 2, 4, 8, "fp64", ngauss=4),
+    1: Config("c1", 8, 16.0, 6, (0.0, 0.0, 0.0), 128, 0, 8, 8, 20, "fp64"),
+    2: Config("c2", 16, 32.0, 6, (0.0, 0.0, 0.0), 512, 0, 64, 8, 24, "fp32"),
+    3: Config("c3", 12, 32.0, 8, (0.25, 0.0, 0.0), 1024, 256, 216, 8, 30, "fp64"),
+    4: Config("c4", 16, 32.0, 6, (0.0, 0.0, 0.0), 512, 0, 64, 8, 24, "fp64"),
+}
+
+CUTOFF = 2.0                 # projector hard cutoff radius, Bohr (config 0; reused for 1-4, A15)
+SIGMA_PROJ = (0.63, 0.9)     # Gaussian radial widths of the two projector shells (A13, A15)
+V_DEPTH, V_WIDTH = -2.0, 1.0  # Gaussian wells: depth (Ha), width (Bohr)
+B_MAG = 0.1                  # |B_xc| in Ha (A14)
+
+
+def tiny_config(ncell=2, p=2, L=4.0, kfrac=(0.0, 0.0, 0.0), nvec=4, natoms=1, nproj=4,
+                degree=6, ngauss=2, name="tiny") -> Config:
+    """A small config for brute-force pins and multi-tile parity cases."""
+    return Config(name, ncell, L, p, tuple(kfrac), nvec, 0, natoms, nproj, degree, "fp64",
+                  ngauss=ngauss)
+
+
+# --------------------------------------------------------------------------- vectors
+def make_vectors(nnodes: int, cols, seed: int = 0) -> np.ndarray:
+    """Complex128 block [nnodes, 2, len(cols)], real and imaginary parts uniform[-1,1].
+
+    Column v is drawn from its own stream `default_rng([seed, v])`, so any subset of the
+    columns of a large block can be produced without generating the rest (columns are
+    independent in the filter).
+    """
+    cols = list(range(cols)) if isinstance(cols, int) else list(cols)
+    X = np.empty((nnodes, 2, len(cols)), dtype=np.complex128)
+    for j, v in enumerate(cols):
+        rng = np.random.default_rng([seed, int(v)])
+        re = rng.uniform(-1.0, 1.0, size=(nnodes, 2))
+        im = rng.uniform(-1.0, 1.0, size=(nnodes, 2))
+        X[:, :, j] = re + 1j * im
+    return X
+
+
+# --------------------------------------------------------------------------- geometry
+def atom_positions(cfg: Config, seed: int = 0) -> np.ndarray:
+    """[natoms,3] positions in [0,L)^3.  Config 0: seeded uniform; else jittered lattice."""
+    rng = np.random.default_rng([seed, 101])
+    if cfg.ngauss > 0:                       # config-0 style: free seeded positions
+        return rng.uniform(0.0, cfg.L, size=(cfg.natoms, 3))
+    na = round(cfg.natoms ** (1.0 / 3.0))
+    if na ** 3 != cfg.natoms:
+        raise ValueError("jittered lattice needs a cubic atom count")
+    a = cfg.L / na
+    g = (np.arange(na) + 0.5) * a
+    zz, yy, xx = np.meshgrid(g, g, g, indexing="ij")
+    pos = np.stack([xx.ravel(), yy.ravel(), zz.ravel()], axis=1)
+    pos = pos + rng.uniform(-0.1 * a, 0.1 * a, size=pos.shape)
+    return np.mod(pos, cfg.L)
+
+
+def gaussian_centres(cfg: Config, atoms: np.ndarray, seed: int = 0) -> np.ndarray:
+    if cfg.ngauss > 0:
+        rng = np.random.default_rng([seed, 102])
+        return rng.uniform(0.0, cfg.L, size=(cfg.ngauss, 3))
+    return atoms.copy()
+
+
+def _min_image(d: np.ndarray, L: float):
+    """Minimum-image displacement and the integer lattice shift n with d_min = d + n*L."""
+    n = -np.rint(d / L)
+    return d + n * L, n
+
+
+# --------------------------------------------------------------------------- local fields
+def local_fields(cfg: Config, xyz: np.ndarray, centres: np.ndarray):
+    """V, Bx, By, Bz at the node coordinates `xyz` [M,3] (supplied by the caller).
+
+    V = sum of periodic Gaussian wells (27 images; width 1 Bohr so farther images are
+    < 1e-13 of the depth for L >= 8); B = 0.1 (0, cos 2 pi x/L, sin 2 pi x/L)  (A14, A15).
+    """
+    M = xyz.shape[0]
+    V = np.zeros(M)
+    shifts = np.array([(i, j, k) for i in (-1, 0, 1) for j in (-1, 0, 1) for k in (-1, 0, 1)],
+                      dtype=np.float64) * cfg.L
+    for c in centres:
+        # only the nearest image matters beyond round-off, but sum all 27 as the recipe says
+        d0 = xyz - c[None, :]
+        for s in shifts:
+            d = d0 - s[None, :]
+            r2 = np.einsum("ij,ij->i", d, d)
+            V += V_DEPTH * np.exp(-r2 / (2.0 * V_WIDTH ** 2))
+    ang = 2.0 * math.pi * xyz[:, 0] / cfg.L
+    Bx = np.zeros(M)
+    By = B_MAG * np.cos(ang)
+    Bz = B_MAG * np.sin(ang)
+    return V, Bx, By, Bz
+
+
+# --------------------------------------------------------------------------- nonlocal
+def projector_tables(cfg: Config, xyz: np.ndarray, atoms: np.ndarray, cutoff: float = CUTOFF):
+    """Support lists and projector values for `chfsi_ham_set`.
+
+    Returns (supp_off [natoms+1] int64, supp_node [nnz] int64, nproj [natoms] int32,
+             P [nnz_rows..] complex128 stored atom after atom, row-major [n_supp_a, nproj_a]).
+    P[I,beta] = beta_shape(r_I + T_I - R_a) * exp(-i k.T_I), T_I the lattice vector of the
+    minimum image; shapes: exp(-r^2/2 sigma^2) x {1, x, y, z},
+    analytically normalised over all space, hard cutoff at `cutoff`.
+    """
+    L = cfg.L
+    kfrac = np.asarray(cfg.kfrac, dtype=np.float64)
+    supp_off = [0]
+    supp_nodes = []
+    P_rows = []
+    nshell = cfg.nproj // 4
+    for Ra in atoms:
+        d, n = _min_image(xyz - Ra[None, :], L)
+        r2 = np.einsum("ij,ij->i", d, d)
+        idx = np.nonzero(r2 < cutoff ** 2)[0]
+        dd, nn, rr2 = d[idx], n[idx], r2[idx]
+        # T_I = n * L; exp(-i k.T) with k = kfrac * 2 pi / L  =>  exp(-2 pi i kfrac.n)
+        phase = np.exp(-2j * math.pi * (nn @ kfrac))
+        cols = []
+        for s in range(nshell):
+            sg = SIGMA_PROJ[s]
+            g = np.exp(-rr2 / (2.0 * sg ** 2))
+            ns = (math.pi * sg ** 2) ** -0.75                    # || exp(-r^2/2sg^2) ||_2 = 1
+            npx = ns * math.sqrt(2.0) / sg                        # || x exp(..) ||_2 = 1
+            cols += [ns * g, npx * dd[:, 0] * g, npx * dd[:, 1] * g, npx * dd[:, 2] * g]
+        Pa = np.stack(cols, axis=1).astype(np.complex128) * phase[:, None]
+        supp_nodes.append(idx.astype(np.int64))
+        P_rows.append(Pa)
+        supp_off.append(supp_off[-1] + idx.size)
+    supp_off = np.asarray(supp_off, dtype=np.int64)
+    supp_node = np.concatenate(supp_nodes) if supp_nodes else np.zeros(0, np.int64)
+    nproj = np.full(len(atoms), cfg.nproj, dtype=np.int32)
+    P = np.concatenate([p.reshape(-1) for p in P_rows]) if P_rows else np.zeros(0, np.complex128)
+    return supp_off, supp_node, nproj, P
+
+
+def soc_couplings(cfg: Config, seed: int = 0) -> np.ndarray:
+    """Per atom a Hermitian (2 nproj)x(2 nproj) complex D_a = Q diag(u) Q^H, u~U[-1,1] Ha (A16).
+
+    Index of a row/column is 2*beta + s (projector beta, spin s).  Returned [natoms, 2np, 2np].
+    """
+    n = 2 * cfg.nproj
+    out = np.empty((cfg.natoms, n, n), dtype=np.complex128)
+    for a in range(cfg.natoms):
+        rng = np.random.default_rng([seed, 103, a])
+        G = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+        Q, _ = np.linalg.qr(G)
+        u = rng.uniform(-1.0, 1.0, size=n)
+        D = (Q * u[None, :]) @ Q.conj().T
+        out[a] = 0.5 * (D + D.conj().T)
+    return out
+
+
+@dataclasses.dataclass
+class HamInputs:
+    V: np.ndarray
+    Bx: np.ndarray
+    By: np.ndarray
+    Bz: np.ndarray
+    atoms: np.ndarray
+    supp_off: np.ndarray
+    supp_node: np.ndarray
+    nproj: np.ndarray
+    P: np.ndarray          # complex128, concatenated per-atom [n_supp_a, nproj_a] row-major
+    D: np.ndarray          # complex128 [natoms, 2 nproj, 2 nproj]
+
+
+def make_hamiltonian(cfg: Config, xyz: np.ndarray, seed: int = 0, with_local=True,
+                     with_nonlocal=True) -> HamInputs:
+    """All `chfsi_ham_set` inputs for a config, sampled at the caller's node coordinates."""
+    atoms = atom_positions(cfg, seed)
+    M = xyz.shape[0]
+    if with_local:
+        V, Bx, By, Bz = local_fields(cfg, xyz, gaussian_centres(cfg, atoms, seed))
+    else:
+        V = np.zeros(M); Bx = np.zeros(M); By = np.zeros(M); Bz = np.zeros(M)
+    if with_nonlocal and cfg.natoms > 0:
+        supp_off, supp_node, nproj, P = projector_tables(cfg, xyz, atoms)
+        D = soc_couplings(cfg, seed)
+    else:
+        atoms = atoms[:0]
+        supp_off = np.zeros(1, np.int64); supp_node = np.zeros(0, np.int64)
+        nproj = np.zeros(0, np.int32); P = np.zeros(0, np.complex128)
+        D = np.zeros((0, 2 * cfg.nproj, 2 * cfg.nproj), np.complex128)
+    return HamInputs(V, Bx, By, Bz, atoms, supp_off, supp_node, nproj, P, D)
+
+
+def lanczos_start(nnodes: int, seed: int = 0) -> np.ndarray:
+    """Seeded start vector [nnodes,2,1] for the harness/oracle Lanczos bound estimate (A4)."""
+    rng = np.random.default_rng([seed, 104])
+    return (rng.standard_normal((nnodes, 2, 1)) + 1j * rng.standard_normal((nnodes, 2, 1)))
