@@ -1,0 +1,146 @@
+/* chfsi.h -- C ABI of the B200 (sm_100a) Chebyshev-filter hot path of R-ChFSI
+ * (arxiv/paper_2605_30128; PAPER.md = the paper text; section/equation numbers are the paper's).
+ *
+ * The library applies  M^-1 H  matrix-free to blocks of complex two-component spinors on a
+ * periodic, uniform, hexahedral, degree-p GLL spectral-element mesh, and runs the paper's
+ * Chebyshev recurrences on top of it:
+ *     H = -1/2 Laplacian + V I + B.sigma + H_nloc                  (eqs. 4, 7)
+ *     discretised as in Sec. III-A (eq. 8) with GLL collocation, so that the
+ *     mass matrix M is diagonal ("D" of PAPER.md:119; BASELINE.json north_star).
+ *
+ * Conventions common to every call
+ *   - Every function returns a chfsi_status; none throws, aborts or prints.
+ *     chfsi_last_error() returns a thread-local, human-readable description of the last failure.
+ *   - "host" pointers are ordinary CPU memory, copied before the call returns (the caller keeps
+ *     ownership).  "device" pointers are CUDA device memory of the mesh's device, owned by the
+ *     caller (e.g. torch tensors); the library never frees or retains them.
+ *   - Multivector layout ("M_{2I+alpha,2J+beta}"): complex128 interleaved (re,im),
+ *     row = 2*I + alpha (node I, spin alpha in {0,1}), vectors fastest:
+ *         X[(2*I + alpha) * ld + v],  0 <= v < nvec <= ld,   ld counted in complex elements.
+ *     Node I = (iz*N1y + iy)*N1x + ix with N1d = ncd * p nodes per direction; node coordinates
+ *     x = (e + (xi_a + 1)/2) * h  for cell e and GLL node xi_a, a = 0..p-1.
+ *   - chfsi_apply_H and chfsi_cheb_filter allocate nothing, never synchronise the host with the
+ *     device, and enqueue all work on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  Setup calls (mesh_create, ham_set, destroy) may allocate and
+ *     synchronise.
+ *   - I/O multivectors are complex128 whatever `prec` is: FP64<->FP32 conversion is fused into the
+ *     kernels' loads and stores (north_star item 5; PAPER.md:208 describes the FP32 operands).
+ */
+#ifndef CHFSI_H
+#define CHFSI_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct chfsi_mesh chfsi_mesh;   /* opaque; owns all device-side operator data */
+
+typedef enum {
+    CHFSI_OK = 0,
+    CHFSI_EINVAL = 1,        /* bad argument (see each call) */
+    CHFSI_ENOMEM = 2,        /* host or device allocation failed */
+    CHFSI_ECUDA = 3,         /* a CUDA runtime call failed; see chfsi_last_error() */
+    CHFSI_ESTATE = 4,        /* call out of order (apply before ham_set) */
+    CHFSI_EUNSUPPORTED = 5   /* no kernel instantiated for this p / precision */
+} chfsi_status;
+
+/* Precision of the H.X product inside the recurrence ("FP32 or TF32").
+ * The recurrence itself, the residual R and Lambda_k are always FP64. */
+typedef enum {
+    CHFSI_FP64 = 0,
+    CHFSI_FP32 = 1,
+    CHFSI_TF32 = 2,          /* reserved: returns CHFSI_EUNSUPPORTED in this build */
+    CHFSI_TF32X3 = 3         /* reserved: returns CHFSI_EUNSUPPORTED in this build */
+} chfsi_prec;
+
+typedef enum {
+    CHFSI_RECUR_STANDARD = 0,   /* eq. 10 */
+    CHFSI_RECUR_RESIDUAL = 1    /* eq. 11, R-ChFSI */
+} chfsi_recur;
+
+/* ---- mesh -------------------------------------------------------------------------------
+ * Periodic box [0,Lx)x[0,Ly)x[0,Lz) cut into ncx*ncy*ncz equal hexahedral cells, FE degree p on
+ * GLL nodes.  kfrac (host, 3 doubles, may be NULL = Gamma) gives the Bloch vector
+ * k_d = kfrac_d * 2 pi / L_d: psi(r + L_d e_d) = exp(2 pi i kfrac_d) psi(r); cell-local nodes
+ * that wrap around the box carry that phase (the paper is silent on k-points; reading O4).
+ * Builds the GLL tables, the diagonal mass m_I and its FP32 copy on `device`.
+ * EINVAL: nc* < 1, L* <= 0, p < 1, out == NULL.  EUNSUPPORTED: p not in {1..8}.  ECUDA/ENOMEM. */
+chfsi_status chfsi_mesh_create(int ncx, int ncy, int ncz, double Lx, double Ly, double Lz, int p,
+                               const double* kfrac, int device, chfsi_mesh** out);
+chfsi_status chfsi_mesh_destroy(chfsi_mesh* mesh);          /* NULL is allowed */
+
+/* Queries (host outputs).  nnodes = M = N1x*N1y*N1z.  xyz: M*3 doubles (x,y,z per node).
+ * mass: M doubles, m_I = sum over the cells containing node I of w_a w_b w_c (hx hy hz / 8). */
+chfsi_status chfsi_mesh_num_nodes(const chfsi_mesh* mesh, long long* nnodes);
+chfsi_status chfsi_mesh_node_coords(const chfsi_mesh* mesh, double* xyz);
+chfsi_status chfsi_mesh_mass(const chfsi_mesh* mesh, double* mass);
+
+/* ---- Hamiltonian data -------------------------------------------------------------------
+ * Local part (eq. 4; spin blocks of eq. 12, pointwise under GLL collocation):
+ *   V, Bx, By, Bz: host, M doubles each (NULL = zero field): V_eff and B_xc at the nodes, Hartree.
+ * Nonlocal part (eq. 7; cell-level projectors and SOC coefficient matrices of
+ * PAPER.md:204):  H_nl = M P D P^H M,
+ *   natoms >= 0; supp_off: host, natoms+1 offsets into supp_node; supp_node: host, node indices
+ *   of each atom's support (each node at most once per atom); nproj: host, natoms projector
+ *   counts (1..16); P_re / P_im: host, for atom a a row-major [n_supp_a][nproj_a] block, blocks
+ *   concatenated in atom order (P_im NULL = real projectors); any Bloch phase exp(-i k.T) of a
+ *   periodic image is already folded into P by the caller.
+ *   D: host, per atom a Hermitian (2 nproj_a)^2 complex matrix, interleaved (re,im), row-major,
+ *   row/column index 2*beta + s (projector beta, spin s); matrices concatenated in atom order.
+ * FP32 copies of all operator data are made here ("single device-to-device cast").
+ * May be called again to replace the Hamiltonian.  EINVAL: support node out of range, bad
+ * offsets, nproj out of range, NULL where data is required. */
+chfsi_status chfsi_ham_set(chfsi_mesh* mesh, const double* V, const double* Bx, const double* By,
+                           const double* Bz, int natoms, const long long* supp_off,
+                           const long long* supp_node, const int* nproj, const double* P_re,
+                           const double* P_im, const double* D);
+
+/* ---- workspace --------------------------------------------------------------------------
+ * Bytes of device scratch `work` needed by chfsi_cheb_filter(prec, recur, chunk) (and, with
+ * recur = CHFSI_RECUR_STANDARD, an upper bound for chfsi_apply_H with nvec <= chunk).
+ * The pointer passed as `work` must be 256-byte aligned. */
+chfsi_status chfsi_workspace_bytes(const chfsi_mesh* mesh, chfsi_prec prec, chfsi_recur recur,
+                                   int chunk, size_t* bytes);
+
+/* ---- Y = M^-1 H X  (one Hamiltonian-multivector product, then D^-1) -----
+ * X, Y: device, complex128, distinct buffers, layout above with leading dimensions ldx, ldy.
+ * prec FP32: X is rounded to FP32 on load, the cell Laplacian and the projector contractions run
+ * in FP32, the result is widened on store.  EINVAL: nvec < 1, ld < nvec, NULL, work too small or
+ * misaligned, X == Y.  ESTATE: before chfsi_ham_set. */
+chfsi_status chfsi_apply_H(const chfsi_mesh* mesh, chfsi_prec prec, int nvec, const void* X,
+                           long long ldx, void* Y, long long ldy, void* work, size_t work_bytes,
+                           void* cuda_stream);
+
+/* ---- Y = C_m(M^-1 H) X  (Chebyshev filter of degree m = `degree`) --------
+ * a = lambda_T (lower edge of the damped interval), b = lambda_max, a0 = lambda_min:
+ * c = (a+b)/2, e = (b-a)/2, sigma_1 = e/(a0-c), sigma_{k+1} = 1/(2/sigma_1 - sigma_k).
+ * recur STANDARD: eq. 10, Y_0 = X, Y_1 = sigma_1 (M^-1 H - c) X / e; lambda_host is ignored.
+ * recur RESIDUAL: eq. 11 with D = M: R = H X - M X Lambda in FP64, Z_0 = 0, Z_1 = sigma_1 R / e,
+ *   Lambda_k by the same recurrence in FP64 on the host, Y = D^-1 Z_m + X Lambda_m;
+ *   lambda_host: host, nvec Ritz values (any finite numbers are legal: with D = M the exact
+ *   result does not depend on them).  With prec FP32 only the product H D^-1 Z_k is inexact;
+ *   R, Z_k, Lambda_k and the four-term combination stay FP64.
+ * The output is Y_m after m applications of H (m = 1 returns Y_1).
+ * chunk = N_b > 0: vectors are processed in blocks of N_b columns ("N_b
+ * wavefunctions"), chunk = 0: all at once.  Y may alias X exactly (same pointer and ld).
+ * EINVAL: degree < 1, b <= a, a0 >= a, nvec < 1, ld < nvec, chunk < 0, chunk % 4 != 0 when
+ * 0 < chunk < nvec, NULL pointers, lambda_host NULL with RESIDUAL, work too small
+ * or misaligned.  ESTATE: before chfsi_ham_set. */
+chfsi_status chfsi_cheb_filter(const chfsi_mesh* mesh, chfsi_prec prec, chfsi_recur recur,
+                               int degree, double a, double b, double a0, int nvec, int chunk,
+                               const void* X, long long ldx, const double* lambda_host, void* Y,
+                               long long ldy, void* work, size_t work_bytes, void* cuda_stream);
+
+/* Number of kernel launches (and memset/memcpy nodes) enqueued by this thread's last successful
+ * chfsi_apply_H / chfsi_cheb_filter call; used by bench.py for its `gpu_launches` claim. */
+long long chfsi_last_launch_count(void);
+
+const char* chfsi_last_error(void);     /* thread-local; never NULL */
+const char* chfsi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHFSI_H */

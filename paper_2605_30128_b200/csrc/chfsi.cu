@@ -1,0 +1,535 @@
+// libchfsi: C-ABI entry points, mesh/Hamiltonian setup and the Chebyshev filter driver.
+// See include/chfsi.h for the contract of every call and DESIGN.md for the data layout.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "chfsi_internal.h"
+
+namespace chfsi {
+
+static thread_local std::string g_err = "";
+static thread_local long long g_launches = 0;
+void set_error(const std::string& s) { g_err = s; }
+void count_launch(int n) { g_launches += n; }
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            set_error(std::string(#call) + ": " + cudaGetErrorString(e_));                         \
+            return e_ == cudaErrorMemoryAllocation ? CHFSI_ENOMEM : CHFSI_ECUDA;                   \
+        }                                                                                          \
+    } while (0)
+
+static chfsi_status fail(chfsi_status st, const std::string& msg) { set_error(msg); return st; }
+
+// ---------------------------------------------------------------------------------------------
+// GLL tables.  Own implementation (shares nothing with oracle/): Newton on P_p' from
+// Chebyshev-Lobatto guesses; derivative matrix from the Legendre closed form
+//   D_ij = P_p(x_i) / (P_p(x_j) (x_i - x_j)), D_00 = -p(p+1)/4, D_pp = p(p+1)/4, D_ii = 0 otherwise.
+static void legendre_pd(int p, double x, double& P, double& dP) {
+    double p0 = 1.0, p1 = x;
+    if (p == 0) { P = 1.0; dP = 0.0; return; }
+    for (int k = 1; k < p; ++k) { const double p2 = ((2 * k + 1) * x * p1 - k * p0) / (k + 1); p0 = p1; p1 = p2; }
+    P = p1;
+    dP = (x * x == 1.0) ? 0.0 : p * (p0 - x * p1) / (1.0 - x * x);
+}
+
+static void gll_tables(int p, std::vector<double>& x, std::vector<double>& w, std::vector<double>& Khat) {
+    const int n = p + 1;
+    x.assign(n, 0.0); w.assign(n, 0.0);
+    x[0] = -1.0; x[p] = 1.0;
+    for (int i = 1; i < p; ++i) {
+        double xi = -std::cos(M_PI * i / p);
+        for (int it = 0; it < 100; ++it) {
+            double P, dP; legendre_pd(p, xi, P, dP);
+            const double d2 = (2.0 * xi * dP - p * (p + 1.0) * P) / (1.0 - xi * xi);
+            const double dx = dP / d2;
+            xi -= dx;
+            if (std::fabs(dx) < 1e-16) break;
+        }
+        x[i] = xi;
+    }
+    for (int i = 0; i < n / 2; ++i) { const double s = 0.5 * (x[p - i] - x[i]); x[i] = -s; x[p - i] = s; }
+    if (n % 2) x[p / 2] = 0.0;
+    std::vector<double> Pv(n);
+    for (int i = 0; i < n; ++i) { double dP; legendre_pd(p, x[i], Pv[i], dP); w[i] = 2.0 / (p * (p + 1.0) * Pv[i] * Pv[i]); }
+    std::vector<double> D(n * n, 0.0);
+    for (int i = 0; i < n; ++i)
+        for (int j = 0; j < n; ++j)
+            if (i != j) D[i * n + j] = Pv[i] / (Pv[j] * (x[i] - x[j]));
+    D[0] = -p * (p + 1.0) / 4.0;
+    D[p * n + p] = p * (p + 1.0) / 4.0;
+    Khat.assign(n * n, 0.0);
+    for (int i = 0; i < n; ++i)
+        for (int j = 0; j < n; ++j) {
+            double s = 0.0;
+            for (int q = 0; q < n; ++q) s += D[q * n + i] * w[q] * D[q * n + j];
+            Khat[i * n + j] = s;
+        }
+    for (int i = 0; i < n; ++i)      // exact symmetry
+        for (int j = i + 1; j < n; ++j) { const double s = 0.5 * (Khat[i * n + j] + Khat[j * n + i]); Khat[i * n + j] = Khat[j * n + i] = s; }
+}
+
+template <typename T>
+static cudaError_t upload(T** dst, const std::vector<T>& src) {
+    *dst = nullptr;
+    if (src.empty()) return cudaSuccess;
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(dst), src.size() * sizeof(T));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+static void free_nonlocal(NonlocalDev& nl) {
+    cudaFree(nl.items); cudaFree(nl.supp_node); cudaFree(nl.supp_mass); cudaFree(nl.p_off); cudaFree(nl.s_off);
+    cudaFree(nl.nproj); cudaFree(nl.c_off); cudaFree(nl.d_off); cudaFree(nl.P64); cudaFree(nl.P32); cudaFree(nl.D64);
+    nl = NonlocalDev();
+}
+
+static double node_mass(const chfsi_mesh* m, long long I) {
+    const long long n1x = m->mc.n1[0], n1y = m->mc.n1[1];
+    const int ix = (int)(I % n1x), iy = (int)((I / n1x) % n1y), iz = (int)(I / (n1x * n1y));
+    return m->mc.m1[0][ix % m->p] * m->mc.m1[1][iy % m->p] * m->mc.m1[2][iz % m->p];
+}
+
+static size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
+
+// workspace layout: [coef table][Cbuf][nbuf multivector buffers]
+struct WorkLayout {
+    size_t hdr_bytes, coef_bytes, c_bytes, buf_bytes, total;
+    int nbuf;
+};
+static WorkLayout work_layout(const chfsi_mesh* m, chfsi_recur recur, int chunk, int degree_cap) {
+    WorkLayout wl;
+    wl.nbuf = recur == CHFSI_RECUR_RESIDUAL ? 3 : 1;
+    wl.hdr_bytes = align256((size_t)(4 + 9 * (degree_cap + 2) + chunk) * sizeof(double));
+    wl.coef_bytes = align256((size_t)(degree_cap + 2) * 2 * chunk * sizeof(double));
+    wl.c_bytes = align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * chunk * 16);
+    wl.buf_bytes = align256((size_t)2 * m->nnodes * chunk * 16);
+    wl.total = wl.hdr_bytes + wl.coef_bytes + wl.c_bytes + wl.nbuf * wl.buf_bytes;
+    return wl;
+}
+constexpr int kDegreeCap = 1024;   // coefficient table is sized for degree <= kDegreeCap
+
+}  // namespace chfsi
+
+using namespace chfsi;
+
+// =============================================================================================
+extern "C" {
+
+const char* chfsi_last_error(void) { return g_err.c_str(); }
+const char* chfsi_version(void) { return "chfsi-b200 0.1 (sm_100a)"; }
+long long chfsi_last_launch_count(void) { return g_launches; }
+
+chfsi_status chfsi_mesh_create(int ncx, int ncy, int ncz, double Lx, double Ly, double Lz, int p,
+                               const double* kfrac, int device, chfsi_mesh** out) {
+    if (out == nullptr) return fail(CHFSI_EINVAL, "mesh_create: out is NULL");
+    *out = nullptr;
+    if (ncx < 1 || ncy < 1 || ncz < 1) return fail(CHFSI_EINVAL, "mesh_create: cells per direction must be >= 1");
+    if (!(Lx > 0) || !(Ly > 0) || !(Lz > 0)) return fail(CHFSI_EINVAL, "mesh_create: box lengths must be > 0");
+    if (p < 1) return fail(CHFSI_EINVAL, "mesh_create: p must be >= 1");
+    if (p > 8) return fail(CHFSI_EUNSUPPORTED, "mesh_create: kernels are instantiated for p <= 8");
+    int ndev = 0;
+    CU(cudaGetDeviceCount(&ndev));
+    if (device < 0 || device >= ndev) return fail(CHFSI_EINVAL, "mesh_create: no such CUDA device");
+    chfsi_mesh* m = new (std::nothrow) chfsi_mesh();
+    if (!m) return fail(CHFSI_ENOMEM, "mesh_create: host allocation failed");
+    m->device = device; m->p = p;
+    m->nc[0] = ncx; m->nc[1] = ncy; m->nc[2] = ncz;
+    m->L[0] = Lx; m->L[1] = Ly; m->L[2] = Lz;
+    for (int d = 0; d < 3; ++d) m->kfrac[d] = kfrac ? kfrac[d] : 0.0;
+    std::vector<double> Khat;
+    gll_tables(p, m->xi, m->w, Khat);
+    MeshConst& mc = m->mc;
+    std::memset(&mc, 0, sizeof(mc));
+    const int n = p + 1;
+    mc.p = p; mc.n = n;
+    double h[3], jac = 1.0;
+    for (int d = 0; d < 3; ++d) {
+        mc.nc[d] = m->nc[d]; mc.n1[d] = m->nc[d] * p;
+        h[d] = m->L[d] / m->nc[d];
+        jac *= 0.5 * h[d];
+    }
+    mc.ncells = ncx * ncy * ncz;
+    mc.nnodes = (long long)mc.n1[0] * mc.n1[1] * mc.n1[2];
+    m->nnodes = mc.nnodes;
+    mc.has_phase = 0;
+    for (int d = 0; d < 3; ++d) {
+        const double fr = m->kfrac[d] - std::floor(m->kfrac[d]);
+        if (fr != 0.0) mc.has_phase = 1;
+        mc.ph_re[d] = fr == 0.0 ? 1.0 : std::cos(2.0 * M_PI * fr);
+        mc.ph_im[d] = fr == 0.0 ? 0.0 : std::sin(2.0 * M_PI * fr);
+        // exact values at the quarter points so that kfrac = 0.25 gives phi = i exactly
+        if (fr == 0.25) { mc.ph_re[d] = 0.0; mc.ph_im[d] = 1.0; }
+        if (fr == 0.5) { mc.ph_re[d] = -1.0; mc.ph_im[d] = 0.0; }
+        if (fr == 0.75) { mc.ph_re[d] = 0.0; mc.ph_im[d] = -1.0; }
+        const double sc = 0.5 * jac * (2.0 / h[d]) * (2.0 / h[d]);
+        for (int i = 0; i < n; ++i)
+            for (int a = 0; a < n; ++a) {
+                mc.Kd[d][i][a] = sc * Khat[i * n + a];
+                mc.Kf[d][i][a] = (float)mc.Kd[d][i][a];
+            }
+        for (int a = 0; a < n; ++a) {
+            const double wa = (a == 0 || a == p) ? 2.0 * m->w[0] : m->w[a];
+            mc.m1[d][a] = 0.5 * h[d] * wa;
+            mc.im1[d][a] = 1.0 / mc.m1[d][a];
+        }
+    }
+    for (int a = 0; a < n; ++a) { mc.w[a] = m->w[a]; mc.wf[a] = (float)m->w[a]; }
+    *out = m;
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
+    if (!m) return CHFSI_OK;
+    {
+        DeviceGuard g(m->device);
+        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz);
+        free_nonlocal(m->nl);
+    }
+    delete m;
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_mesh_num_nodes(const chfsi_mesh* m, long long* nnodes) {
+    if (!m || !nnodes) return fail(CHFSI_EINVAL, "mesh_num_nodes: NULL argument");
+    *nnodes = m->nnodes;
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_mesh_node_coords(const chfsi_mesh* m, double* xyz) {
+    if (!m || !xyz) return fail(CHFSI_EINVAL, "mesh_node_coords: NULL argument");
+    const int p = m->p;
+    std::vector<double> line[3];
+    for (int d = 0; d < 3; ++d) {
+        const double h = m->L[d] / m->nc[d];
+        line[d].resize(m->mc.n1[d]);
+        for (int e = 0; e < m->nc[d]; ++e)
+            for (int a = 0; a < p; ++a) line[d][e * p + a] = e * h + 0.5 * (m->xi[a] + 1.0) * h;
+    }
+    long long I = 0;
+    for (int iz = 0; iz < m->mc.n1[2]; ++iz)
+        for (int iy = 0; iy < m->mc.n1[1]; ++iy)
+            for (int ix = 0; ix < m->mc.n1[0]; ++ix, ++I) {
+                xyz[3 * I + 0] = line[0][ix]; xyz[3 * I + 1] = line[1][iy]; xyz[3 * I + 2] = line[2][iz];
+            }
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_mesh_mass(const chfsi_mesh* m, double* mass) {
+    if (!m || !mass) return fail(CHFSI_EINVAL, "mesh_mass: NULL argument");
+    for (long long I = 0; I < m->nnodes; ++I) mass[I] = node_mass(m, I);
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, const double* By,
+                           const double* Bz, int natoms, const long long* supp_off,
+                           const long long* supp_node, const int* nproj, const double* P_re,
+                           const double* P_im, const double* D) {
+    if (!m) return fail(CHFSI_EINVAL, "ham_set: mesh is NULL");
+    if (natoms < 0) return fail(CHFSI_EINVAL, "ham_set: natoms < 0");
+    if (natoms > 0 && (!supp_off || !nproj || !D)) return fail(CHFSI_EINVAL, "ham_set: NULL nonlocal table");
+    const long long M = m->nnodes;
+    // ---- validate the nonlocal tables on the host first
+    long long nnz = 0, pcount = 0, dcount = 0, crows = 0;
+    int max_np = 0;
+    std::vector<long long> p_off(natoms), d_off(natoms), c_off(natoms), s_off(natoms + 1, 0);
+    for (int a = 0; a < natoms; ++a) {
+        if (nproj[a] < 1 || nproj[a] > kMaxProj) return fail(CHFSI_EINVAL, "ham_set: nproj must be in 1..16");
+        const long long ns = supp_off[a + 1] - supp_off[a];
+        if (ns < 0 || supp_off[0] != 0) return fail(CHFSI_EINVAL, "ham_set: supp_off must start at 0 and be non-decreasing");
+        p_off[a] = pcount; d_off[a] = dcount; c_off[a] = crows; s_off[a + 1] = supp_off[a + 1];
+        pcount += ns * nproj[a];
+        dcount += 4ll * nproj[a] * nproj[a];
+        crows += 2 * nproj[a];
+        nnz += ns;
+        if (nproj[a] > max_np) max_np = nproj[a];
+    }
+    if (nnz > 0 && (!supp_node || !P_re)) return fail(CHFSI_EINVAL, "ham_set: NULL support list or projector values");
+    for (long long j = 0; j < nnz; ++j)
+        if (supp_node[j] < 0 || supp_node[j] >= M) return fail(CHFSI_EINVAL, "ham_set: support node out of range");
+    DeviceGuard g(m->device);
+    if (!g.ok) return fail(CHFSI_ECUDA, "ham_set: cannot select device");
+    // ---- local fields
+    std::vector<double> zero;
+    const double* src[4] = {V, Bx, By, Bz};
+    double** dst[4] = {&m->dV, &m->dBx, &m->dBy, &m->dBz};
+    for (int f = 0; f < 4; ++f) {
+        if (*dst[f] == nullptr) CU(cudaMalloc(reinterpret_cast<void**>(dst[f]), M * sizeof(double)));
+        if (src[f]) CU(cudaMemcpy(*dst[f], src[f], M * sizeof(double), cudaMemcpyHostToDevice));
+        else CU(cudaMemset(*dst[f], 0, M * sizeof(double)));
+    }
+    m->mc.V = m->dV; m->mc.Bx = m->dBx; m->mc.By = m->dBy; m->mc.Bz = m->dBz;
+    // ---- nonlocal tables
+    free_nonlocal(m->nl);
+    NonlocalDev& nl = m->nl;
+    nl.natoms = natoms; nl.nnz = nnz; nl.max_nproj = max_np; nl.crows = crows;
+    if (natoms > 0 && nnz > 0) {
+        std::vector<ProjItem> items;
+        constexpr int kSlice = 64;
+        for (int a = 0; a < natoms; ++a) {
+            const long long ns = supp_off[a + 1] - supp_off[a];
+            for (long long st = 0; st < ns; st += kSlice)
+                items.push_back(ProjItem{a, (int)st, (int)((ns - st) < kSlice ? (ns - st) : kSlice)});
+        }
+        nl.nitems = (int)items.size();
+        std::vector<long long> nodes(supp_node, supp_node + nnz);
+        std::vector<double> smass(nnz);
+        for (long long j = 0; j < nnz; ++j) smass[j] = node_mass(m, nodes[j]);
+        std::vector<double2> P64(pcount);
+        std::vector<float2> P32(pcount);
+        for (long long j = 0; j < pcount; ++j) {
+            P64[j] = make_double2(P_re[j], P_im ? P_im[j] : 0.0);
+            P32[j] = make_float2((float)P64[j].x, (float)P64[j].y);
+        }
+        std::vector<double2> D64(dcount);
+        for (long long j = 0; j < dcount; ++j) D64[j] = make_double2(D[2 * j], D[2 * j + 1]);
+        std::vector<int> np(nproj, nproj + natoms);
+        CU(upload(&nl.items, items));
+        CU(upload(&nl.supp_node, nodes));
+        CU(upload(&nl.supp_mass, smass));
+        CU(upload(&nl.p_off, p_off));
+        CU(upload(&nl.s_off, s_off));
+        CU(upload(&nl.nproj, np));
+        CU(upload(&nl.c_off, c_off));
+        CU(upload(&nl.d_off, d_off));
+        CU(upload(&nl.P64, P64));
+        CU(upload(&nl.P32, P32));
+        CU(upload(&nl.D64, D64));
+    }
+    CU(cudaDeviceSynchronize());
+    m->ham_set = true;
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_workspace_bytes(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur recur, int chunk, size_t* bytes) {
+    if (!m || !bytes) return fail(CHFSI_EINVAL, "workspace_bytes: NULL argument");
+    if (chunk < 1) return fail(CHFSI_EINVAL, "workspace_bytes: chunk must be >= 1");
+    if (recur != CHFSI_RECUR_STANDARD && recur != CHFSI_RECUR_RESIDUAL) return fail(CHFSI_EINVAL, "workspace_bytes: bad recur");
+    if (!cell_supported(m->p, prec)) return fail(CHFSI_EUNSUPPORTED, "workspace_bytes: precision not built");
+    *bytes = work_layout(m, recur, chunk, kDegreeCap).total;
+    return CHFSI_OK;
+}
+
+// One accumulation  out += cH * s_out * H(s_in * in) + cin * f * in + cR * R  : projector forward pass,
+// cell kernel, projector back pass.  `out` must already hold the value being accumulated into.
+static chfsi_status accumulate_H(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& ca, double* Cbuf, cudaStream_t st) {
+    const bool nlocal = m->nl.nitems > 0;
+    if (nlocal) {
+        CU(cudaMemsetAsync(Cbuf, 0, (size_t)m->nl.crows * ca.nvec * 16, st));
+        count_launch();
+        ProjArgs pa{ca.in, ca.ld_in, Cbuf, ca.nvec, (ca.flags & kScaleIn) ? 0 : 1};
+        CU(launch_proj(m, prec, pa, st));
+    }
+    CU(launch_cell(m, prec, ca, st));
+    if (nlocal) {
+        BackArgs ba{Cbuf, ca.out, ca.ld_out, ca.cH, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
+        CU(launch_back(m, prec, ba, st));
+    }
+    return CHFSI_OK;
+}
+
+static chfsi_status check_common(const chfsi_mesh* m, chfsi_prec prec, int nvec, const void* X, long long ldx,
+                                 const void* Y, long long ldy, const void* work, const char* who) {
+    if (!m) return fail(CHFSI_EINVAL, std::string(who) + ": mesh is NULL");
+    if (!m->ham_set) return fail(CHFSI_ESTATE, std::string(who) + ": chfsi_ham_set has not been called");
+    if (prec == CHFSI_TF32 || prec == CHFSI_TF32X3) return fail(CHFSI_EUNSUPPORTED, std::string(who) + ": TF32 paths are not built");
+    if (!cell_supported(m->p, prec)) return fail(CHFSI_EUNSUPPORTED, std::string(who) + ": precision/degree not built");
+    if (nvec < 1) return fail(CHFSI_EINVAL, std::string(who) + ": nvec must be >= 1");
+    if (!X || !Y || !work) return fail(CHFSI_EINVAL, std::string(who) + ": NULL device pointer");
+    if (ldx < nvec || ldy < nvec) return fail(CHFSI_EINVAL, std::string(who) + ": leading dimension < nvec");
+    if (((uintptr_t)work & 255) != 0) return fail(CHFSI_EINVAL, std::string(who) + ": work must be 256-byte aligned");
+    if (((uintptr_t)X & 15) != 0 || ((uintptr_t)Y & 15) != 0) return fail(CHFSI_EINVAL, std::string(who) + ": X and Y must be 16-byte aligned");
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_apply_H(const chfsi_mesh* m, chfsi_prec prec, int nvec, const void* X, long long ldx,
+                           void* Y, long long ldy, void* work, size_t work_bytes, void* cuda_stream) {
+    chfsi_status stt = check_common(m, prec, nvec, X, ldx, Y, ldy, work, "apply_H");
+    if (stt != CHFSI_OK) return stt;
+    if (X == Y) return fail(CHFSI_EINVAL, "apply_H: X and Y must be distinct");
+    const size_t need = align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * nvec * 16);
+    if (work_bytes < need) return fail(CHFSI_EINVAL, "apply_H: work_bytes too small");
+    DeviceGuard g(m->device);
+    if (!g.ok) return fail(CHFSI_ECUDA, "apply_H: cannot select device");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    g_launches = 0;
+    CU(cudaMemset2DAsync(Y, (size_t)ldy * 16, 0, (size_t)nvec * 16, (size_t)2 * m->nnodes, st));
+    count_launch();
+    CellArgs ca{};
+    ca.in = static_cast<const double*>(X); ca.ld_in = ldx;
+    ca.out = static_cast<double*>(Y); ca.ld_out = ldy;
+    ca.R = nullptr; ca.ld_R = 0; ca.cin = nullptr; ca.cR = nullptr;
+    ca.cH = 1.0; ca.nvec = nvec; ca.flags = kSoutInvM;
+    return accumulate_H(m, prec, ca, static_cast<double*>(work), st);
+}
+
+chfsi_status chfsi_cheb_filter(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur recur, int degree,
+                               double a, double b, double a0, int nvec, int chunk, const void* X,
+                               long long ldx, const double* lambda_host, void* Y, long long ldy,
+                               void* work, size_t work_bytes, void* cuda_stream) {
+    chfsi_status stt = check_common(m, prec, nvec, X, ldx, Y, ldy, work, "cheb_filter");
+    if (stt != CHFSI_OK) return stt;
+    if (recur != CHFSI_RECUR_STANDARD && recur != CHFSI_RECUR_RESIDUAL) return fail(CHFSI_EINVAL, "cheb_filter: bad recur");
+    if (degree < 1 || degree > kDegreeCap) return fail(CHFSI_EINVAL, "cheb_filter: degree must be in 1..1024");
+    if (!(b > a)) return fail(CHFSI_EINVAL, "cheb_filter: need b > a");
+    if (!(a0 < a)) return fail(CHFSI_EINVAL, "cheb_filter: need a0 < a");
+    if (chunk < 0) return fail(CHFSI_EINVAL, "cheb_filter: chunk < 0");
+    if (chunk == 0 || chunk > nvec) chunk = nvec;
+    if (chunk < nvec && chunk % 4 != 0) return fail(CHFSI_EINVAL, "cheb_filter: chunk must be a multiple of 4");
+    if (recur == CHFSI_RECUR_RESIDUAL && !lambda_host) return fail(CHFSI_EINVAL, "cheb_filter: lambda_host is NULL");
+    if (X == Y && ldx != ldy) return fail(CHFSI_EINVAL, "cheb_filter: aliased X/Y need equal leading dimensions");
+    const WorkLayout wl = work_layout(m, recur, chunk, kDegreeCap);
+    if (work_bytes < wl.total) return fail(CHFSI_EINVAL, "cheb_filter: work_bytes too small");
+    DeviceGuard g(m->device);
+    if (!g.ok) return fail(CHFSI_ECUDA, "cheb_filter: cannot select device");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    g_launches = 0;
+
+    // ---- scalars of PAPER.md:119
+    const double c = 0.5 * (b + a), e = 0.5 * (b - a);
+    std::vector<double> sig(degree + 2, 0.0);
+    sig[1] = e / (a0 - c);
+    for (int k = 1; k < degree; ++k) sig[k + 1] = 1.0 / (2.0 / sig[1] - sig[k]);
+    auto alpha = [&](int k) { return 2.0 * sig[k + 1] / e; };
+    auto beta = [&](int k) { return 2.0 * sig[k + 1] * c / e; };
+    auto gamma = [&](int k) { return sig[k] * sig[k + 1]; };
+
+    char* wbase = static_cast<char*>(work);
+    double* dhdr = reinterpret_cast<double*>(wbase);
+    double* coef = reinterpret_cast<double*>(wbase + wl.hdr_bytes);
+    double* Cbuf = reinterpret_cast<double*>(wbase + wl.hdr_bytes + wl.coef_bytes);
+    double* buf[3];
+    for (int i = 0; i < 3; ++i)
+        buf[i] = reinterpret_cast<double*>(wbase + wl.hdr_bytes + wl.coef_bytes + wl.c_bytes + (size_t)i * wl.buf_bytes);
+    const size_t bufbytes_used = (size_t)2 * m->nnodes * 16;   // per column
+
+    for (int j0 = 0; j0 < nvec; j0 += chunk) {
+        const int nb = (nvec - j0) < chunk ? (nvec - j0) : chunk;
+        const double* Xc = static_cast<const double*>(X) + 2ll * j0;
+        double* Yc = static_cast<double*>(Y) + 2ll * j0;
+        // Row program for this chunk (a few KB, inlined in the command stream); the per-vector table,
+        // including the FP64 Lambda_k recurrence, is built on the device by coef_kernel.
+        const int nrows = degree + 1;
+        std::vector<CoefRow> rows(nrows, CoefRow{0, 0, 0, 0, 0, 0, 0, 0, 0});
+        auto dCIN = [&](int r) { return coef + (size_t)r * 2 * nb; };
+        auto dCR = [&](int r) { return coef + (size_t)r * 2 * nb + nb; };
+        auto upload_rows = [&](double q0, double q1, const double* lam) -> chfsi_status {
+            std::vector<double> hdr(4 + 9 * (size_t)nrows + nb, 0.0);
+            hdr[0] = q0; hdr[1] = q1; hdr[2] = nrows;
+            std::memcpy(hdr.data() + 4, rows.data(), sizeof(CoefRow) * nrows);
+            if (lam) std::memcpy(hdr.data() + 4 + 9 * (size_t)nrows, lam, sizeof(double) * nb);
+            CU(cudaMemcpyAsync(dhdr, hdr.data(), hdr.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+            count_launch();
+            CU(launch_coef(dhdr, coef, nrows, nb, st));
+            return CHFSI_OK;
+        };
+
+        if (recur == CHFSI_RECUR_RESIDUAL) {
+            // In-place accumulation: stored Zh_k = Z_k / s_k with s_{k+1} = -gamma_k s_{k-1}, so that
+            //   Zh_{k+1} = Zh_{k-1} + (s_k/s_{k+1}) [alpha_k H D^-1 Zh_k - beta_k Zh_k] + (alpha_k/s_{k+1}) R Lambda_k
+            // is a pure "+=" into the buffer that holds Zh_{k-1} ("in-place recurrence").
+            // s_1 = sigma_1/e makes Zh_1 = R exactly, so R's buffer doubles as Zh_1.
+            std::vector<double> s(degree + 2, 1.0);
+            s[0] = 1.0; s[1] = sig[1] / e;
+            for (int k = 1; k < degree; ++k) s[k + 1] = -gamma(k) * s[k - 1];
+            // row 0: S0, cin = -lambda_v (carries m_I in the kernel); rows 1..m-1: the steps; row m: recover
+            rows[0].cinLam = -1.0;
+            std::vector<double> cHs(degree + 1, 0.0);
+            for (int k = 1; k < degree; ++k) {
+                const double r = s[k] / s[k + 1];
+                cHs[k] = r * alpha(k);
+                CoefRow& rw = rows[k];
+                rw.cin0 = -r * beta(k);
+                if (k == 1) rw.cinL = alpha(k) / s[k + 1];      // in == R at the first step: R-term folded into cin
+                else rw.cRL = alpha(k) / s[k + 1];
+                if (k == 2) rw.cR0 = 1.0;                        // Zh_1 = R: the "+= Zh_{k-1}" term, folded in
+                rw.al = alpha(k); rw.be = beta(k); rw.ga = gamma(k); rw.advance = 1.0;
+            }
+            rows[degree].cin0 = s[degree];                       // recover: Y = (s_m / m) Zh_m + Lambda_m X
+            rows[degree].cRL = 1.0;
+            stt = upload_rows(-sig[1] * c / e, sig[1] / e, lambda_host + j0);   // Lambda_1 = sigma_1 (lambda - c)/e
+            if (stt != CHFSI_OK) return stt;
+            double* R = buf[0];
+            double* Zb[2] = {buf[1], buf[2]};
+            CU(cudaMemsetAsync(R, 0, bufbytes_used * nb, st)); count_launch();
+            // S0: R = H X - M X Lambda (FP64 always, Alg. 1 line 3)
+            CellArgs ca{};
+            ca.in = Xc; ca.ld_in = ldx; ca.out = R; ca.ld_out = nb; ca.R = nullptr; ca.ld_R = 0;
+            ca.cin = dCIN(0); ca.cR = nullptr; ca.cH = 1.0; ca.nvec = nb; ca.flags = kMassIn;
+            stt = accumulate_H(m, CHFSI_FP64, ca, Cbuf, st);
+            if (stt != CHFSI_OK) return stt;
+            const double* zin = R;       // Zh_1
+            double* zcur = R;
+            for (int k = 1; k < degree; ++k) {
+                double* zout;
+                if (k == 1) zout = Zb[0];
+                else if (k == 2) zout = Zb[1];
+                else zout = (k % 2 == 1) ? Zb[0] : Zb[1];   // Zh_{k+1} overwrites Zh_{k-1}
+                if (k <= 2) { CU(cudaMemsetAsync(zout, 0, bufbytes_used * nb, st)); count_launch(); }
+                CellArgs cs{};
+                cs.in = zin; cs.ld_in = nb; cs.out = zout; cs.ld_out = nb;
+                cs.R = (k >= 2) ? R : nullptr; cs.ld_R = nb;
+                cs.cin = dCIN(k); cs.cR = (k >= 2) ? dCR(k) : nullptr;
+                cs.cH = cHs[k]; cs.nvec = nb; cs.flags = kScaleIn;
+                stt = accumulate_H(m, prec, cs, Cbuf, st);
+                if (stt != CHFSI_OK) return stt;
+                zin = zout; zcur = zout;
+            }
+            // S7 recover: Y = D^-1 Z_m + X Lambda_m
+            CU(launch_axpby(m, Yc, ldy, zcur, nb, dCIN(degree), 1, Xc, ldx, dCR(degree), nb, st));
+        } else {
+            // eq. 10 with the same in-place trick: Yh_k = Y_k / s_k, s_{k+1} = -gamma_k s_{k-1}, and the chain
+            // with the parity of m normalised so that s_m = 1: the last accumulation lands in Y unscaled.
+            std::vector<double> s(degree + 2, 1.0);
+            for (int k = 1; k < degree; ++k) s[k + 1] = -gamma(k) * s[k - 1];
+            const double sm = s[degree];
+            for (int k = degree; k >= 0; k -= 2) s[k] /= sm;
+            // buffers: even indices live in E, odd in O; the one with the parity of m is Y itself
+            double* Wb = buf[0];
+            double* E = (degree % 2 == 0) ? Yc : Wb;  long long ldE = (degree % 2 == 0) ? ldy : nb;
+            double* O = (degree % 2 == 0) ? Wb : Yc;  long long ldO = (degree % 2 == 0) ? nb : ldy;
+            // row 0: scaled copy Yh_0 = X / s_0 ; row k+1: cin of step k (uniform over vectors)
+            rows[0].cin0 = 1.0 / s[0];
+            // step 0 (Y_1 = sigma_1 (M^-1 H - c) X / e):  Yh_1 = (s_0/s_1)(sigma_1/e) [M^-1 H Yh_0 - c Yh_0]
+            std::vector<double> cHs(degree + 1, 0.0);
+            cHs[0] = (s[0] / s[1]) * sig[1] / e;
+            rows[1].cin0 = -cHs[0] * c;
+            for (int k = 1; k < degree; ++k) {
+                const double r = s[k] / s[k + 1];
+                cHs[k] = r * alpha(k);
+                rows[k + 1].cin0 = -r * beta(k);
+            }
+            stt = upload_rows(0.0, 0.0, nullptr);
+            if (stt != CHFSI_OK) return stt;
+            CU(launch_axpby(m, E, ldE, Xc, ldx, dCIN(0), 0, nullptr, 0, nullptr, nb, st));   // E = X / s_0 (in place if E aliases X)
+            CU(cudaMemset2DAsync(O, (size_t)ldO * 16, 0, (size_t)nb * 16, (size_t)2 * m->nnodes, st)); count_launch();
+            for (int k = 0; k < degree; ++k) {
+                const bool in_even = (k % 2 == 0);
+                CellArgs cs{};
+                cs.in = in_even ? E : O; cs.ld_in = in_even ? ldE : ldO;
+                cs.out = in_even ? O : E; cs.ld_out = in_even ? ldO : ldE;
+                cs.R = nullptr; cs.ld_R = 0; cs.cin = dCIN(k + 1); cs.cR = nullptr;
+                cs.cH = cHs[k]; cs.nvec = nb; cs.flags = kSoutInvM;
+                stt = accumulate_H(m, prec, cs, Cbuf, st);
+                if (stt != CHFSI_OK) return stt;
+            }
+        }
+    }
+    return CHFSI_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,131 @@
+// Internal declarations of libchfsi (sm_100a).  Not part of the C ABI (include/chfsi.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "chfsi.h"
+
+namespace chfsi {
+
+constexpr int kMaxN = 9;        // p + 1 <= 9  (p <= 8)
+constexpr int kMaxProj = 16;    // projectors per atom
+
+// Everything a kernel needs to know about the mesh; passed by value (__grid_constant__), so the
+// 1-D matrices sit in the constant bank and become immediate operands of the unrolled FMAs.
+struct MeshConst {
+    int p, n;                   // degree, n = p + 1
+    int nc[3];                  // cells per direction
+    int n1[3];                  // nodes per direction
+    int ncells;
+    int has_phase;              // any kfrac != integer
+    long long nnodes;
+    double Kd[3][kMaxN][kMaxN]; // 0.5 * J * (2/h_d)^2 * Khat[i][a]   (kinetic 1/2 folded in)
+    float  Kf[3][kMaxN][kMaxN];
+    double w[kMaxN];            // GLL weights
+    float  wf[kMaxN];
+    double m1[3][kMaxN];        // assembled 1-D mass at cell-local index a: (h_d/2) * (w_a, doubled on faces)
+    double im1[3][kMaxN];       // reciprocals
+    double ph_re[3], ph_im[3];  // Bloch phases phi_d = exp(2 pi i kfrac_d)
+    const double* V;            // node fields (device), never null after ham_set
+    const double* Bx;
+    const double* By;
+    const double* Bz;
+};
+
+enum CellFlags : int {
+    kScaleIn = 1,     // w = in / m      (Z-form of eq. 11: H D^-1 Z)
+    kSoutInvM = 2,    // multiply H w by 1/m   (M^-1 H, eq. 10 and chfsi_apply_H)
+    kMassIn = 4,      // the in-term carries m_I  (residual R = H X - M X Lambda)
+};
+
+// out += cH * s_out * H(s_in * in) + cin[v] * f * in + cR[v] * R      (accumulated with RED.ADD.F64)
+struct CellArgs {
+    const double* in;  long long ld_in;     // leading dimensions in complex elements
+    double* out;       long long ld_out;
+    const double* R;   long long ld_R;      // nullptr: no R term
+    const double* cin;                      // [nvec] per-vector coefficient of the in-term (device)
+    const double* cR;                       // [nvec] per-vector coefficient of the R-term (device) or nullptr
+    double cH;
+    int nvec;
+    int flags;
+};
+
+struct ProjItem { int atom; int start; int count; };   // a slice of an atom's support list
+
+struct NonlocalDev {
+    int natoms = 0;
+    int nitems = 0;
+    int max_nproj = 0;
+    long long nnz = 0;                  // total support entries
+    ProjItem* items = nullptr;          // [nitems]
+    long long* supp_node = nullptr;     // [nnz]
+    double* supp_mass = nullptr;        // [nnz] m_I of each support entry
+    long long* p_off = nullptr;         // [natoms] offset (in complex elements) of atom's P block
+    long long* s_off = nullptr;         // [natoms+1] support offsets
+    int* nproj = nullptr;               // [natoms]
+    long long* c_off = nullptr;         // [natoms] offset of atom's coefficient rows in Cbuf (units of rows)
+    long long* d_off = nullptr;         // [natoms] offset of atom's D matrix (complex elements)
+    double2* P64 = nullptr;             // complex128 projector values
+    float2* P32 = nullptr;
+    double2* D64 = nullptr;
+    long long crows = 0;                // sum over atoms of 2*nproj  (rows of Cbuf)
+};
+
+struct ProjArgs {
+    const double* in; long long ld_in;
+    double* C;                          // [crows][nvec] complex128, zeroed by the driver
+    int nvec;
+    int mass_u;                         // 1: u = m_I * in (apply on X); 0: u = in (Z-form)
+};
+
+struct BackArgs {
+    const double* C;                    // projected coefficients
+    double* out; long long ld_out;
+    double cH;
+    int nvec;
+    int sout_invm;                      // 1: s_out = 1/m  => m * (1/m) = 1 ; 0: factor m_I
+};
+
+}  // namespace chfsi
+
+struct chfsi_mesh {
+    int device = 0;
+    int p = 0;
+    int nc[3] = {0, 0, 0};
+    double L[3] = {0, 0, 0};
+    double kfrac[3] = {0, 0, 0};
+    long long nnodes = 0;
+    bool ham_set = false;
+    chfsi::MeshConst mc;
+    std::vector<double> xi, w;          // host GLL tables
+    std::vector<double> m1h[3];         // host assembled 1-D mass per global line index
+    double* dV = nullptr;
+    double* dBx = nullptr;
+    double* dBy = nullptr;
+    double* dBz = nullptr;
+    chfsi::NonlocalDev nl;
+};
+
+namespace chfsi {
+// launchers (kernels.cu)
+cudaError_t launch_cell(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
+cudaError_t launch_proj(const chfsi_mesh* m, chfsi_prec prec, const ProjArgs& a, cudaStream_t s);
+cudaError_t launch_back(const chfsi_mesh* m, chfsi_prec prec, const BackArgs& a, cudaStream_t s);
+// out[row][v] = ca[v] * (inv_mass ? A/m : A) + cb[v] * B   (B, cb may be null); rows = 2*nnodes
+cudaError_t launch_axpby(const chfsi_mesh* m, double* out, long long ldo, const double* A, long long lda,
+                         const double* ca, int a_inv_mass, const double* B, long long ldb,
+                         const double* cb, int nvec, cudaStream_t s);
+// Per-step coefficient rows.  For vector v with Ritz value lam and the running Lambda_k(v) = L:
+//   cin[r][v] = cin0 + cinL * L + cinLam * lam ;  cR[r][v] = cR0 + cRL * L ;
+//   then, if advance: L_next = al * lam * L - be * L - ga * L_prev   (Lambda_k recurrence)
+struct CoefRow { double cin0, cinL, cinLam, cR0, cRL, al, be, ga, advance; };
+// hdr (device): [q0, q1, nrows, pad] then nrows CoefRow, then lam[nvec]; L_0 = 1, L_1 = q0 + q1 * lam.
+// table (device): row r = [cin(0..nvec-1), cR(0..nvec-1)]
+cudaError_t launch_coef(const double* hdr, double* table, int nrows, int nvec, cudaStream_t s);
+bool cell_supported(int p, chfsi_prec prec);
+void set_error(const std::string& s);
+void count_launch(int n = 1);
+}  // namespace chfsi

@@ -1,0 +1,422 @@
+// sm_100a kernels of libchfsi: cell gather / sum-factorised Laplacian / fused pointwise update with
+// in-place L2 reductions (S1-S3, S5, S6 of DESIGN.md), nonlocal projector kernels (S4), and the
+// pointwise recover/scale kernel (S7).
+#include "chfsi_internal.h"
+
+namespace chfsi {
+
+// ---------------------------------------------------------------------------------------------
+// helpers
+template <typename TT> struct KSel;
+template <> struct KSel<double> {
+    static __device__ __forceinline__ double K(const MeshConst& mc, int d, int i, int a) { return mc.Kd[d][i][a]; }
+    static __device__ __forceinline__ double w(const MeshConst& mc, int a) { return mc.w[a]; }
+};
+template <> struct KSel<float> {
+    static __device__ __forceinline__ float K(const MeshConst& mc, int d, int i, int a) { return mc.Kf[d][i][a]; }
+    static __device__ __forceinline__ float w(const MeshConst& mc, int a) { return mc.wf[a]; }
+};
+
+__device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }  // result unused -> RED.E.ADD.F64
+
+// ---------------------------------------------------------------------------------------------
+// Cell kernel.  One CTA = one FE cell x NV complex vectors (C = 4 NV real batch columns: re/im of both
+// spin components, which the spin-diagonal real Laplacian treats alike -- north_star kernel (1)/(2)).
+//   S1 gather   : W^(e) = R^(e) (s_in * in)           (PAPER.md:204 stage (i); Bloch phase on wrapped nodes)
+//   S2 Laplacian: T^(e) = 1/2 K_e W^(e) by three 1-D contractions
+//                 pass 1: each thread owns one xy-plane of one column, x- and y-contractions in registers
+//                 pass 2: each thread owns z-lines, z-contraction in registers, straight into the epilogue
+//   S3 assembly : out[I] += conj(phase) * cH * s_out * T^(e)   (RED.ADD.F64 at L2; PAPER.md:204 stage (iii))
+//   S5 pointwise: on the nodes the cell owns (local index < p in every direction) the 2x2 spin
+//                 potential of eq. 12, the in-term and the R-term of eq. 11 are added in the same pass.
+// Thread t: column col = t % C, group grp = t / C, G = n groups.
+template <int P, int NV, typename TT>
+__global__ void __launch_bounds__((P + 1) * 4 * NV)
+cell_kernel(const __grid_constant__ MeshConst mc, const __grid_constant__ CellArgs ar) {
+    constexpr int n = P + 1, n3 = n * n * n, C = 4 * NV, G = n;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TT* W = reinterpret_cast<TT*>(smem_raw);
+    TT* T2 = W + n3 * C;
+
+    const int tid = threadIdx.x;
+    const int col = tid % C, grp = tid / C;
+    const int cell = blockIdx.x % mc.ncells, chunk = blockIdx.x / mc.ncells;
+    const int ex = cell % mc.nc[0], ey = (cell / mc.nc[0]) % mc.nc[1], ez = cell / (mc.nc[0] * mc.nc[1]);
+    const int s = col / (2 * NV), vl = (col % (2 * NV)) >> 1, ri = col & 1;
+    const int v = chunk * NV + vl;
+    const bool vok = v < ar.nvec;
+    const int flags = ar.flags;
+    const bool hasph = mc.has_phase != 0;
+
+    // ---- S1 gather
+    {
+        const double* __restrict__ src = ar.in + ((long long)s * ar.ld_in + v) * 2 + ri;
+        for (int l = grp; l < n3; l += G) {
+            const int a = l % n, b = (l / n) % n, c = l / (n * n);
+            int gx = ex * P + a, gy = ey * P + b, gz = ez * P + c;
+            const bool wx = gx == mc.n1[0], wy = gy == mc.n1[1], wz = gz == mc.n1[2];
+            gx = wx ? 0 : gx; gy = wy ? 0 : gy; gz = wz ? 0 : gz;
+            const long long I = ((long long)gz * mc.n1[1] + gy) * mc.n1[0] + gx;
+            double val = vok ? __ldg(src + I * 4 * ar.ld_in) : 0.0;
+            if (hasph) {
+                const double other = __shfl_xor_sync(__activemask(), val, 1);
+                if (wx | wy | wz) {
+                    double pr = 1.0, pi = 0.0;
+                    if (wx) { pr = mc.ph_re[0]; pi = mc.ph_im[0]; }
+                    if (wy) { const double t = pr * mc.ph_re[1] - pi * mc.ph_im[1]; pi = pr * mc.ph_im[1] + pi * mc.ph_re[1]; pr = t; }
+                    if (wz) { const double t = pr * mc.ph_re[2] - pi * mc.ph_im[2]; pi = pr * mc.ph_im[2] + pi * mc.ph_re[2]; pr = t; }
+                    // (re + i im)(pr + i pi): re' = re pr - im pi ; im' = re pi + im pr
+                    val = ri == 0 ? val * pr - other * pi : other * pi + val * pr;
+                }
+            }
+            if (flags & kScaleIn) val *= mc.im1[0][a] * mc.im1[1][b] * mc.im1[2][c];
+            W[l * C + col] = (TT)val;
+        }
+    }
+    __syncthreads();
+
+    // ---- S2 pass 1: xy-plane c = grp; T2[c][j][i] = w_c ( w_j (Kx W)_i + w_i (Ky W)_j )
+    for (int c = grp; c < n; c += G) {
+        TT o[n][n];
+#pragma unroll
+        for (int j = 0; j < n; ++j)
+#pragma unroll
+            for (int i = 0; i < n; ++i) o[j][i] = (TT)0;
+#pragma unroll
+        for (int b = 0; b < n; ++b) {
+            TT in[n];
+#pragma unroll
+            for (int a = 0; a < n; ++a) in[a] = W[((c * n + b) * n + a) * C + col];
+            const TT wb = KSel<TT>::w(mc, b);
+#pragma unroll
+            for (int i = 0; i < n; ++i) {
+                TT sx = (TT)0;
+#pragma unroll
+                for (int a = 0; a < n; ++a) sx = fma(KSel<TT>::K(mc, 0, i, a), in[a], sx);
+                o[b][i] = fma(wb, sx, o[b][i]);
+            }
+#pragma unroll
+            for (int a = 0; a < n; ++a) {
+                const TT t = KSel<TT>::w(mc, a) * in[a];
+#pragma unroll
+                for (int j = 0; j < n; ++j) o[j][a] = fma(KSel<TT>::K(mc, 1, j, b), t, o[j][a]);
+            }
+        }
+        const TT wc = KSel<TT>::w(mc, c);
+#pragma unroll
+        for (int j = 0; j < n; ++j)
+#pragma unroll
+            for (int i = 0; i < n; ++i) T2[((c * n + j) * n + i) * C + col] = wc * o[j][i];
+    }
+    __syncthreads();
+
+    // ---- S2 pass 2 + S3/S5 epilogue: z-lines (b,a)
+    const double cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
+    const double cR = (vok && ar.cR) ? __ldg(ar.cR + v) : 0.0;
+    const bool useR = ar.R != nullptr && ar.cR != nullptr;
+    for (int li = grp; li < n * n; li += G) {
+        const int a = li % n, b = li / n;
+        TT in[n], t[n];
+#pragma unroll
+        for (int c = 0; c < n; ++c) {
+            in[c] = W[((c * n + b) * n + a) * C + col];
+            t[c] = T2[((c * n + b) * n + a) * C + col];
+        }
+        const TT wab = KSel<TT>::w(mc, a) * KSel<TT>::w(mc, b);
+#pragma unroll
+        for (int k = 0; k < n; ++k) {
+            TT sz = (TT)0;
+#pragma unroll
+            for (int c = 0; c < n; ++c) sz = fma(KSel<TT>::K(mc, 2, k, c), in[c], sz);
+            t[k] = fma(wab, sz, t[k]);
+        }
+        int gx = ex * P + a, gy = ey * P + b;
+        const bool wx = gx == mc.n1[0], wy = gy == mc.n1[1];
+        gx = wx ? 0 : gx; gy = wy ? 0 : gy;
+        const double mab = mc.m1[0][a] * mc.m1[1][b];
+        const double imab = mc.im1[0][a] * mc.im1[1][b];
+#pragma unroll
+        for (int k = 0; k < n; ++k) {
+            int gz = ez * P + k;
+            const bool wz = gz == mc.n1[2];
+            gz = wz ? 0 : gz;
+            const long long I = ((long long)gz * mc.n1[1] + gy) * mc.n1[0] + gx;
+            const double mI = mab * mc.m1[2][k];
+            const double imI = imab * mc.im1[2][k];
+            const double sout = (flags & kSoutInvM) ? imI : 1.0;
+            double val = ar.cH * sout * (double)t[k];
+            if (hasph) {
+                const double other = __shfl_xor_sync(__activemask(), val, 1);
+                if (wx | wy | wz) {
+                    double pr = 1.0, pi = 0.0;
+                    if (wx) { pr = mc.ph_re[0]; pi = mc.ph_im[0]; }
+                    if (wy) { const double tt = pr * mc.ph_re[1] - pi * mc.ph_im[1]; pi = pr * mc.ph_im[1] + pi * mc.ph_re[1]; pr = tt; }
+                    if (wz) { const double tt = pr * mc.ph_re[2] - pi * mc.ph_im[2]; pi = pr * mc.ph_im[2] + pi * mc.ph_re[2]; pr = tt; }
+                    // multiply by conj(phase): re' = re pr + im pi ; im' = im pr - re pi
+                    val = ri == 0 ? val * pr + other * pi : val * pr - other * pi;
+                }
+            }
+            if (a < P && b < P && k < P) {   // node owned by this cell: pointwise terms (never wrapped)
+                const int l = (k * n + b) * n + a;
+                // u = m_I * w for both spins / both parts of this vector.  FP64: recovered from the tile
+                // (one extra rounding); FP32: re-read in FP64 so the recurrence terms stay exact FP64.
+                double u_own, u_oth_re, u_oth_im, in_own;
+                const int ocol = col ^ (2 * NV);            // same vector, other spin
+                if (sizeof(TT) == 8) {
+                    const double f = (flags & kScaleIn) ? mI : 1.0;      // in = w * f
+                    in_own = (double)in[k] * f;
+                    const double o_same = (double)W[l * C + ocol] * f;   // other spin, same part
+                    const double o_flip = (double)W[l * C + (ocol ^ 1)] * f;
+                    u_oth_re = ri == 0 ? o_same : o_flip;
+                    u_oth_im = ri == 0 ? o_flip : o_same;
+                } else {
+                    const double* base = ar.in + I * 4 * ar.ld_in;
+                    in_own = vok ? __ldg(base + ((long long)s * ar.ld_in + v) * 2 + ri) : 0.0;
+                    const double2 oth = vok ? __ldg(reinterpret_cast<const double2*>(base + ((long long)(s ^ 1) * ar.ld_in + v) * 2))
+                                            : make_double2(0.0, 0.0);
+                    u_oth_re = oth.x; u_oth_im = oth.y;
+                }
+                const double fu = (flags & kScaleIn) ? 1.0 : mI;         // u = m w: Z-form u = in, else m * in
+                u_own = in_own * fu;
+                u_oth_re *= fu; u_oth_im *= fu;
+                const double Vn = __ldg(mc.V + I), Bxn = __ldg(mc.Bx + I), Byn = __ldg(mc.By + I), Bzn = __ldg(mc.Bz + I);
+                // eq. 12 spin blocks, pointwise: up: (V+Bz) u_up + (Bx - i By) u_dn ; dn: (Bx + i By) u_up + (V - Bz) u_dn
+                const double diag = s == 0 ? Vn + Bzn : Vn - Bzn;
+                const double sy = s == 0 ? -Byn : Byn;                   // off-diagonal = Bx + i sy
+                // (Bx + i sy)(re + i im) = (Bx re - sy im) + i (Bx im + sy re)
+                const double offd = ri == 0 ? Bxn * u_oth_re - sy * u_oth_im : Bxn * u_oth_im + sy * u_oth_re;
+                val += ar.cH * sout * (diag * u_own + offd);
+                val += cin * ((flags & kMassIn) ? mI : 1.0) * in_own;
+                if (useR && vok) val += cR * __ldg(ar.R + ((2 * I + s) * ar.ld_R + v) * 2 + ri);
+            }
+            if (vok) red_add(ar.out + ((2 * I + s) * ar.ld_out + v) * 2 + ri, val);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S4 forward projection: C_a[2 beta + s][v] += sum_{I in slice} conj(P_a[I,beta]) u_{I,s,v}
+// One CTA = one slice of an atom's support x 128 (spin, vector) columns.
+template <typename TT>
+__global__ void __launch_bounds__(128)
+proj_kernel(const NonlocalDev nl, const ProjArgs ar) {
+    const ProjItem it = nl.items[blockIdx.x];
+    const int s = blockIdx.y & 1;
+    const int v = (blockIdx.y >> 1) * 128 + threadIdx.x;
+    if (v >= ar.nvec) return;
+    const int np = nl.nproj[it.atom];
+    const long long soff = nl.s_off[it.atom];
+    const long long poff = nl.p_off[it.atom];
+    TT acc_re[kMaxProj], acc_im[kMaxProj];
+#pragma unroll
+    for (int b = 0; b < kMaxProj; ++b) { acc_re[b] = 0; acc_im[b] = 0; }
+    for (int jj = 0; jj < it.count; ++jj) {
+        const long long j = it.start + jj;                 // index within the atom's support
+        const long long I = nl.supp_node[soff + j];
+        double2 x = __ldg(reinterpret_cast<const double2*>(ar.in) + (2 * I + s) * ar.ld_in + v);
+        if (ar.mass_u) { const double m = nl.supp_mass[soff + j]; x.x *= m; x.y *= m; }
+        const TT xr = (TT)x.x, xi = (TT)x.y;
+#pragma unroll
+        for (int b = 0; b < kMaxProj; ++b) {
+            if (b < np) {
+                TT pr, pi;
+                if (sizeof(TT) == 8) { const double2 pv = nl.P64[poff + j * np + b]; pr = pv.x; pi = pv.y; }
+                else { const float2 pv = nl.P32[poff + j * np + b]; pr = pv.x; pi = pv.y; }
+                // conj(p) x = (pr - i pi)(xr + i xi)
+                acc_re[b] = fma(pr, xr, fma(pi, xi, acc_re[b]));
+                acc_im[b] = fma(pr, xi, fma(-pi, xr, acc_im[b]));
+            }
+        }
+    }
+    double* Crow = ar.C + (nl.c_off[it.atom] * (long long)ar.nvec + v) * 2;
+#pragma unroll
+    for (int b = 0; b < kMaxProj; ++b) {
+        if (b < np) {
+            double* dst = Crow + (long long)(2 * b + s) * ar.nvec * 2;
+            red_add(dst, (double)acc_re[b]);
+            red_add(dst + 1, (double)acc_im[b]);
+        }
+    }
+}
+
+// S4 back projection: out_{I,s,v} += cH * f_I * sum_beta P_a[I,beta] G_a[2 beta + s][v],  G_a = D_a C_a
+template <typename TT>
+__global__ void __launch_bounds__(128)
+back_kernel(const NonlocalDev nl, const BackArgs ar) {
+    const ProjItem it = nl.items[blockIdx.x];
+    const int s = blockIdx.y & 1;
+    const int v = (blockIdx.y >> 1) * 128 + threadIdx.x;
+    if (v >= ar.nvec) return;
+    const int np = nl.nproj[it.atom];
+    const long long soff = nl.s_off[it.atom];
+    const long long poff = nl.p_off[it.atom];
+    const double2* D = nl.D64 + nl.d_off[it.atom];
+    const double2* Cc = reinterpret_cast<const double2*>(ar.C) + nl.c_off[it.atom] * (long long)ar.nvec + v;
+    TT g_re[kMaxProj], g_im[kMaxProj];
+#pragma unroll
+    for (int b = 0; b < kMaxProj; ++b) {
+        double gr = 0.0, gi = 0.0;
+        if (b < np) {
+            const int row = 2 * b + s;
+            for (int r = 0; r < 2 * np; ++r) {
+                const double2 d = D[row * 2 * np + r];
+                const double2 c = Cc[(long long)r * ar.nvec];
+                gr += d.x * c.x - d.y * c.y;
+                gi += d.x * c.y + d.y * c.x;
+            }
+        }
+        g_re[b] = (TT)gr; g_im[b] = (TT)gi;
+    }
+    for (int jj = 0; jj < it.count; ++jj) {
+        const long long j = it.start + jj;
+        const long long I = nl.supp_node[soff + j];
+        TT yr = 0, yi = 0;
+#pragma unroll
+        for (int b = 0; b < kMaxProj; ++b) {
+            if (b < np) {
+                TT pr, pi;
+                if (sizeof(TT) == 8) { const double2 pv = nl.P64[poff + j * np + b]; pr = pv.x; pi = pv.y; }
+                else { const float2 pv = nl.P32[poff + j * np + b]; pr = pv.x; pi = pv.y; }
+                yr = fma(pr, g_re[b], fma(-pi, g_im[b], yr));
+                yi = fma(pr, g_im[b], fma(pi, g_re[b], yi));
+            }
+        }
+        const double f = ar.cH * (ar.sout_invm ? 1.0 : nl.supp_mass[soff + j]);
+        double* dst = ar.out + ((2 * I + s) * ar.ld_out + v) * 2;
+        red_add(dst, f * (double)yr);
+        red_add(dst + 1, f * (double)yi);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S7 / scaled copies: out[row][v] = ca[v] * (a_inv_mass ? A/m : A) + cb[v] * B
+__global__ void __launch_bounds__(256)
+axpby_kernel(const __grid_constant__ MeshConst mc, double2* __restrict__ out, long long ldo,
+             const double2* __restrict__ A, long long lda, const double* __restrict__ ca, int a_inv_mass,
+             const double2* __restrict__ B, long long ldb, const double* __restrict__ cb, int nvec) {
+    const long long rows = 2 * mc.nnodes;
+    const long long total = rows * nvec;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const long long row = idx / nvec;
+        const int v = (int)(idx - row * nvec);
+        double f = ca[v];
+        if (a_inv_mass) {
+            const long long I = row >> 1;
+            const int ix = (int)(I % mc.n1[0]);
+            const int iy = (int)((I / mc.n1[0]) % mc.n1[1]);
+            const int iz = (int)(I / ((long long)mc.n1[0] * mc.n1[1]));
+            f *= mc.im1[0][ix % mc.p] * mc.im1[1][iy % mc.p] * mc.im1[2][iz % mc.p];
+        }
+        const double2 av = A[row * lda + v];
+        double2 r = make_double2(f * av.x, f * av.y);
+        if (B != nullptr) {
+            const double g = cb[v];
+            const double2 bv = B[row * ldb + v];
+            r.x = fma(g, bv.x, r.x); r.y = fma(g, bv.y, r.y);
+        }
+        out[row * ldo + v] = r;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Coefficient table: one thread per vector runs the FP64 Lambda_k recurrence.
+__global__ void coef_kernel(const double* __restrict__ hdr, double* __restrict__ table, int nrows, int nvec) {
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= nvec) return;
+    const CoefRow* rows = reinterpret_cast<const CoefRow*>(hdr + 4);
+    const double lam = hdr[4 + 9 * (size_t)nrows + v];
+    double Lp = 1.0, L = hdr[0] + hdr[1] * lam;
+    for (int r = 0; r < nrows; ++r) {
+        const CoefRow row = rows[r];
+        table[(size_t)r * 2 * nvec + v] = row.cin0 + row.cinL * L + row.cinLam * lam;
+        table[(size_t)r * 2 * nvec + nvec + v] = row.cR0 + row.cRL * L;
+        if (row.advance != 0.0) {
+            const double Ln = row.al * lam * L - row.be * L - row.ga * Lp;
+            Lp = L; L = Ln;
+        }
+    }
+}
+
+cudaError_t launch_coef(const double* hdr, double* table, int nrows, int nvec, cudaStream_t st) {
+    coef_kernel<<<(nvec + 127) / 128, 128, 0, st>>>(hdr, table, nrows, nvec);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// launchers
+template <int P, int NV, typename TT>
+static cudaError_t launch_cell_t(const chfsi_mesh* m, const CellArgs& a, cudaStream_t st) {
+    constexpr int n = P + 1, C = 4 * NV;
+    const size_t smem = 2ull * n * n * n * C * sizeof(TT);
+    static bool attr_done[64] = {false};
+    auto kern = cell_kernel<P, NV, TT>;
+    if (!attr_done[m->device & 63]) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_done[m->device & 63] = true;
+    }
+    const int nchunks = (a.nvec + NV - 1) / NV;
+    const long long grid = (long long)m->mc.ncells * nchunks;
+    kern<<<(unsigned)grid, n * C, smem, st>>>(m->mc, a);
+    count_launch();
+    return cudaGetLastError();
+}
+
+bool cell_supported(int p, chfsi_prec prec) {
+    if (prec != CHFSI_FP64 && prec != CHFSI_FP32) return false;
+    return p >= 1 && p <= 8;
+}
+
+cudaError_t launch_cell(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t st) {
+    const bool f32 = prec == CHFSI_FP32;
+#define CELL_CASE(PP, NV64, NV32)                                                     \
+    case PP:                                                                           \
+        return f32 ? launch_cell_t<PP, NV32, float>(m, a, st) : launch_cell_t<PP, NV64, double>(m, a, st);
+    switch (m->p) {
+        CELL_CASE(1, 8, 8)
+        CELL_CASE(2, 8, 8)
+        CELL_CASE(3, 8, 8)
+        CELL_CASE(4, 8, 8)
+        CELL_CASE(5, 8, 8)
+        CELL_CASE(6, 4, 8)
+        CELL_CASE(7, 4, 8)
+        CELL_CASE(8, 4, 4)
+        default: return cudaErrorInvalidValue;
+    }
+#undef CELL_CASE
+}
+
+cudaError_t launch_proj(const chfsi_mesh* m, chfsi_prec prec, const ProjArgs& a, cudaStream_t st) {
+    if (m->nl.nitems == 0) return cudaSuccess;
+    dim3 grid(m->nl.nitems, 2 * ((a.nvec + 127) / 128));
+    if (prec == CHFSI_FP32) proj_kernel<float><<<grid, 128, 0, st>>>(m->nl, a);
+    else proj_kernel<double><<<grid, 128, 0, st>>>(m->nl, a);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_back(const chfsi_mesh* m, chfsi_prec prec, const BackArgs& a, cudaStream_t st) {
+    if (m->nl.nitems == 0) return cudaSuccess;
+    dim3 grid(m->nl.nitems, 2 * ((a.nvec + 127) / 128));
+    if (prec == CHFSI_FP32) back_kernel<float><<<grid, 128, 0, st>>>(m->nl, a);
+    else back_kernel<double><<<grid, 128, 0, st>>>(m->nl, a);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_axpby(const chfsi_mesh* m, double* out, long long ldo, const double* A, long long lda,
+                         const double* ca, int a_inv_mass, const double* B, long long ldb,
+                         const double* cb, int nvec, cudaStream_t st) {
+    const long long total = 2 * m->nnodes * (long long)nvec;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    axpby_kernel<<<(unsigned)blocks, 256, 0, st>>>(m->mc, reinterpret_cast<double2*>(out), ldo,
+                                                   reinterpret_cast<const double2*>(A), lda, ca, a_inv_mass,
+                                                   reinterpret_cast<const double2*>(B), ldb, cb, nvec);
+    count_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace chfsi

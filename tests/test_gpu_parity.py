@@ -1,0 +1,230 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances (BASELINE.json north_star): relative Frobenius error 1e-11 per
+filter call in FP64, 1e-5 with the FP32-inexact product.  `-m gpu`.
+"""
+import numpy as np
+import pytest
+
+from paper_2605_30128_b200 import inputs as inp
+
+pytestmark = pytest.mark.gpu
+
+TOL64, TOL32 = 1e-11, 1e-5
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from oracle import fe_oracle as fo
+    from paper_2605_30128_b200 import binding as B
+    B.lib()                                     # fails loudly if the extension is missing
+    return torch, fo, B
+
+
+class Problem:
+    """Same mesh + Hamiltonian on both sides (inputs generated once, from the oracle's coordinates)."""
+
+    def __init__(self, env, cfg, seed=0, with_local=True, with_nonlocal=True):
+        torch, fo, B = env
+        self.torch, self.fo, self.B, self.cfg = torch, fo, B, cfg
+        self.omesh = fo.Mesh(cfg.ncell, cfg.L, cfg.p, cfg.kfrac)
+        self.gmesh = B.chfsi_mesh_create(cfg.ncell, cfg.L, cfg.p, cfg.kfrac, 0)
+        xyz = self.omesh.node_coords()
+        assert B.chfsi_mesh_num_nodes(self.gmesh) == self.omesh.nnodes
+        gx = B.chfsi_mesh_node_coords(self.gmesh)
+        assert np.max(np.abs(gx - xyz)) < 1e-13 * cfg.L
+        gm = B.chfsi_mesh_mass(self.gmesh)
+        assert np.max(np.abs(gm - self.omesh.mass)) < 1e-13 * np.max(gm)
+        hi = inp.make_hamiltonian(cfg, xyz, seed=seed, with_local=with_local, with_nonlocal=with_nonlocal)
+        self.hi = hi
+        self.oham = fo.Hamiltonian(self.omesh, hi.V, hi.Bx, hi.By, hi.Bz, hi.supp_off, hi.supp_node,
+                                   hi.nproj, hi.P, hi.D)
+        if len(hi.supp_off) > 1:
+            B.chfsi_ham_set(self.gmesh, hi.V, hi.Bx, hi.By, hi.Bz, hi.supp_off, hi.supp_node, hi.nproj,
+                            hi.P, hi.D)
+        else:
+            B.chfsi_ham_set(self.gmesh, hi.V, hi.Bx, hi.By, hi.Bz)
+
+    def close(self):
+        self.B.chfsi_mesh_destroy(self.gmesh)
+
+    def work(self, prec, recur, chunk):
+        n = self.B.chfsi_workspace_bytes(self.gmesh, prec, recur, chunk)
+        return self.torch.empty(n, dtype=self.torch.uint8, device="cuda")
+
+    def gpu_apply(self, X, prec):
+        t, B = self.torch, self.B
+        Xd = t.from_numpy(X).cuda()
+        Yd = t.full_like(Xd, float("nan"))
+        B.chfsi_apply_H(self.gmesh, prec, Xd, Yd, self.work(prec, B.RECUR_STANDARD, X.shape[2]))
+        t.cuda.synchronize()
+        return Yd.cpu().numpy()
+
+    def gpu_filter(self, X, lam, degree, a, b, a0, prec, recur, chunk=0, alias=False):
+        t, B = self.torch, self.B
+        Xd = t.from_numpy(X).cuda()
+        Yd = Xd if alias else t.full_like(Xd, float("nan"))
+        nb = chunk if chunk else X.shape[2]
+        B.chfsi_cheb_filter(self.gmesh, prec, recur, degree, a, b, a0, Xd, lam, Yd, self.work(prec, recur, nb),
+                            chunk=chunk)
+        t.cuda.synchronize()
+        return Yd.cpu().numpy()
+
+    def bounds(self, steps=10):
+        a0, b = self.fo.lanczos_bounds(self.oham, inp.lanczos_start(self.omesh.nnodes), steps)
+        return a0 + 0.1 * (b - a0), b, a0
+
+    def rayleigh(self, X):
+        HX = self.fo.apply_H(self.oham, X)
+        num = np.real(np.einsum("isv,isv->v", X.conj(), HX))
+        den = np.real(np.einsum("isv,isv->v", X.conj(), self.omesh.mass[:, None, None] * X))
+        return num / den
+
+
+def relerr(A, B):
+    return float(np.linalg.norm(A - B) / np.linalg.norm(B))
+
+
+# ------------------------------------------------------------------------------- apply_H
+@pytest.mark.parametrize("p,ncell,kfrac,nvec", [
+    (2, 2, (0, 0, 0), 4), (3, 3, (0.25, 0.1, -0.3), 5), (4, 2, (0, 0, 0), 9), (6, 2, (0.25, 0, 0), 12),
+    (8, 2, (0, 0.5, 0), 3), (1, 4, (0.3, 0, 0), 2), (5, 2, (0, 0, 0), 8), (7, 2, (0, 0, 0.25), 4)])
+def test_apply_H_matches_oracle(env, p, ncell, kfrac, nvec):
+    _, fo, B = env
+    cfg = inp.tiny_config(ncell=ncell, p=p, L=2.0 * ncell, kfrac=kfrac, nvec=nvec, natoms=2, nproj=8, ngauss=3)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, nvec)
+        ref = fo.apply_MinvH(pb.oham, X)
+        assert relerr(pb.gpu_apply(X, B.FP64), ref) < 1e-13
+        assert relerr(pb.gpu_apply(X, B.FP32), ref) < 2e-6
+    finally:
+        pb.close()
+
+
+def test_apply_H_terms_separately_and_leading_dimension(env):
+    torch, fo, B = env
+    cfg = inp.tiny_config(ncell=3, p=4, L=6.0, kfrac=(0.25, 0, 0), nvec=6, natoms=1, nproj=4)
+    for wl, wn in [(False, False), (True, False), (False, True)]:
+        pb = Problem(env, cfg, with_local=wl, with_nonlocal=wn)
+        try:
+            X = inp.make_vectors(cfg.nnodes, 6)
+            ref = fo.apply_MinvH(pb.oham, X)
+            # ld > nvec on both sides, nvec not a multiple of the CTA's vector tile
+            Xd = torch.zeros((cfg.nnodes, 2, 11), dtype=torch.complex128, device="cuda")
+            Xd[:, :, :6] = torch.from_numpy(X).cuda()
+            Yd = torch.full((cfg.nnodes, 2, 13), 7.0, dtype=torch.complex128, device="cuda")
+            B.chfsi_apply_H(pb.gmesh, B.FP64, Xd, Yd, pb.work(B.FP64, B.RECUR_STANDARD, 6), nvec=6)
+            torch.cuda.synchronize()
+            Y = Yd.cpu().numpy()
+            assert relerr(Y[:, :, :6], ref) < 1e-13
+            assert np.all(Y[:, :, 6:] == 7.0)                      # padding columns untouched
+        finally:
+            pb.close()
+
+
+# ------------------------------------------------------------------------------- filter, small meshes
+@pytest.mark.parametrize("p,ncell,kfrac,degree", [(2, 2, (0, 0, 0), 9), (4, 3, (0.25, 0, 0), 8), (6, 2, (0, 0, 0), 11),
+                                                  (3, 2, (0.1, 0.2, 0.3), 1), (3, 2, (0, 0, 0), 2), (8, 2, (0.25, 0, 0), 6)])
+def test_filter_fp64_both_recurrences(env, p, ncell, kfrac, degree):
+    _, fo, B = env
+    cfg = inp.tiny_config(ncell=ncell, p=p, L=2.0 * ncell, kfrac=kfrac, nvec=6, natoms=2, nproj=8, ngauss=3)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, 6)
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref10 = fo.cheb_filter_standard(pb.oham, X, degree, a, b, a0)
+        ref11 = fo.cheb_filter_residual(pb.oham, X, lam, degree, a, b, a0)
+        assert relerr(pb.gpu_filter(X, None, degree, a, b, a0, B.FP64, B.RECUR_STANDARD), ref10) < TOL64
+        assert relerr(pb.gpu_filter(X, lam, degree, a, b, a0, B.FP64, B.RECUR_RESIDUAL), ref11) < TOL64
+        # aliased output and arbitrary Lambda (with D = M the exact result does not depend on it, P5)
+        assert relerr(pb.gpu_filter(X, None, degree, a, b, a0, B.FP64, B.RECUR_STANDARD, alias=True), ref10) < TOL64
+        assert relerr(pb.gpu_filter(X, np.zeros(6), degree, a, b, a0, B.FP64, B.RECUR_RESIDUAL, alias=True), ref11) < 1e-10
+    finally:
+        pb.close()
+
+
+def test_filter_fp32_inexact_product(env):
+    _, fo, B = env
+    cfg = inp.tiny_config(ncell=3, p=4, L=6.0, kfrac=(0.25, 0, 0), nvec=8, natoms=2, nproj=8, ngauss=3)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, 8)
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref = fo.cheb_filter_residual(pb.oham, X, lam, 12, a, b, a0)
+        e11 = relerr(pb.gpu_filter(X, lam, 12, a, b, a0, B.FP32, B.RECUR_RESIDUAL), ref)
+        e10 = relerr(pb.gpu_filter(X, None, 12, a, b, a0, B.FP32, B.RECUR_STANDARD), ref)
+        assert 1e-9 < e11 < TOL32 and e10 < TOL32          # inexact, but within the stated tolerance
+    finally:
+        pb.close()
+
+
+def test_filter_chunked_equals_unchunked_and_ragged(env):
+    _, fo, B = env
+    cfg = inp.tiny_config(ncell=2, p=4, L=4.0, nvec=11, natoms=1, nproj=4)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, 11)
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref = fo.cheb_filter_residual(pb.oham, X, lam, 7, a, b, a0)
+        full = pb.gpu_filter(X, lam, 7, a, b, a0, B.FP64, B.RECUR_RESIDUAL)
+        chunked = pb.gpu_filter(X, lam, 7, a, b, a0, B.FP64, B.RECUR_RESIDUAL, chunk=4)   # 4 + 4 + 3
+        assert relerr(full, ref) < TOL64 and relerr(chunked, ref) < TOL64
+        ch10 = pb.gpu_filter(X, None, 7, a, b, a0, B.FP64, B.RECUR_STANDARD, chunk=8)
+        assert relerr(ch10, ref) < TOL64
+    finally:
+        pb.close()
+
+
+# ------------------------------------------------------------------------------- BASELINE configs
+def test_config0_full(env):
+    """configs[0]: 4^3 cells, p=4, Gamma, 16 vectors, degree 8, bounds from a 10-step Lanczos; full block."""
+    _, fo, B = env
+    cfg = inp.CONFIGS[0]
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, cfg.nvec, seed=0)
+        a, b, a0 = pb.bounds(10)
+        lam = pb.rayleigh(X)
+        ref = fo.cheb_filter_residual(pb.oham, X, lam, cfg.degree, a, b, a0)
+        assert relerr(pb.gpu_filter(X, lam, cfg.degree, a, b, a0, B.FP64, B.RECUR_RESIDUAL), ref) < TOL64
+        assert relerr(pb.gpu_filter(X, None, cfg.degree, a, b, a0, B.FP64, B.RECUR_STANDARD), ref) < TOL64
+        assert relerr(pb.gpu_filter(X, lam, cfg.degree, a, b, a0, B.FP32, B.RECUR_RESIDUAL), ref) < TOL32
+    finally:
+        pb.close()
+
+
+def _sampled_config_case(env, cfg, cols, precs, nvec_gpu, chunk=0):
+    """Run the GPU on a block of nvec_gpu columns that contains the sampled columns `cols` of the
+    config's seeded block; run the oracle on the sampled columns only (columns are independent, P12)."""
+    torch, fo, B = env
+    pb = Problem(env, cfg)
+    try:
+        allcols = list(range(nvec_gpu))
+        X = inp.make_vectors(cfg.nnodes, allcols, seed=0)
+        Xs = X[:, :, cols]
+        a, b, a0 = pb.bounds(10)
+        lam_s = pb.rayleigh(Xs)
+        lam = np.zeros(nvec_gpu)
+        lam[cols] = lam_s
+        ref = fo.cheb_filter_residual(pb.oham, Xs, lam_s, cfg.degree, a, b, a0)
+        out = {}
+        for prec, tol in precs:
+            Y = pb.gpu_filter(X, lam, cfg.degree, a, b, a0, prec, B.RECUR_RESIDUAL, chunk=chunk)
+            out[prec] = relerr(Y[:, :, cols], ref)
+            assert out[prec] < tol, (prec, out[prec])
+        return out
+    finally:
+        pb.close()
+
+
+def test_config1_full_size_sampled_columns(env):
+    """configs[1] at full size in the launch configuration bench.py times (128 vectors, degree 20, FP64):
+    oracle on 3 sampled columns."""
+    _, _, B = env
+    _sampled_config_case(env, inp.CONFIGS[1], [0, 77, 127], [(B.FP64, TOL64), (B.FP32, TOL32)], 128)
