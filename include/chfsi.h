@@ -137,6 +137,18 @@ chfsi_status chfsi_cheb_filter(const chfsi_mesh* mesh, chfsi_prec prec, chfsi_re
  * chfsi_apply_H / chfsi_cheb_filter call; used by bench.py for its `gpu_launches` claim. */
 long long chfsi_last_launch_count(void);
 
+/* ---- profiling aid (bench.py's roofline block) --------------------------------------------
+ * While enabled, every launch of the dominant kernel (the cell kernel: gather + sum-factorised
+ * Laplacian + fused assembly/pointwise/recurrence update) is bracketed by CUDA events on the stream
+ * it is launched on.  chfsi_profile_read synchronises on those events, returns the summed duration
+ * (ms), the number of launches and the summed ALGORITHMIC bytes of those launches -- per unit
+ * (complex DoF x vector): 16 B for each multivector read (in; R when the step uses it) plus 32 B for
+ * the read-modify-write of the accumulated output, i.e. 64 B for an eq. 11 step with k >= 2 and
+ * 48 B for eq. 10 steps, the residual S0 and the first eq. 11 step -- and clears the record. */
+chfsi_status chfsi_profile_enable(chfsi_mesh* mesh, int on);
+chfsi_status chfsi_profile_read(chfsi_mesh* mesh, double* cell_ms, long long* cell_launches,
+                                double* cell_alg_bytes);
+
 const char* chfsi_last_error(void);     /* thread-local; never NULL */
 const char* chfsi_version(void);
 

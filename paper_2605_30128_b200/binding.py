@@ -23,6 +23,7 @@ PREC = {"fp64": FP64, "fp32": FP32, "tf32": TF32, "tf32x3": TF32X3}
 EXPORTS = [
     "chfsi_mesh_create", "chfsi_mesh_destroy", "chfsi_mesh_num_nodes", "chfsi_mesh_node_coords",
     "chfsi_mesh_mass", "chfsi_ham_set", "chfsi_workspace_bytes", "chfsi_apply_H", "chfsi_cheb_filter",
+    "chfsi_profile_enable", "chfsi_profile_read",
     "chfsi_last_launch_count", "chfsi_last_error", "chfsi_version",
 ]
 
@@ -56,7 +57,9 @@ def lib() -> C.CDLL:
     L.chfsi_cheb_filter.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                     C.c_int, C.c_int, vp, C.c_longlong, dp, vp, C.c_longlong, vp,
                                     C.c_size_t, vp]
-    for name in EXPORTS[:9]:
+    L.chfsi_profile_enable.argtypes = [vp, C.c_int]
+    L.chfsi_profile_read.argtypes = [vp, dp, llp, dp]
+    for name in EXPORTS[:11]:
         getattr(L, name).restype = C.c_int
     L.chfsi_last_launch_count.restype = C.c_longlong
     L.chfsi_last_error.restype = C.c_char_p
@@ -167,6 +170,17 @@ def chfsi_cheb_filter(mesh, prec, recur, degree, a, b, a0, X, lam, Y, work, chun
     _check(lib().chfsi_cheb_filter(mesh, int(prec), int(recur), int(degree), float(a), float(b), float(a0),
                                    int(nvec), int(chunk), _ptr(X), int(ldx), _dptr(lam_h), _ptr(Y), int(ldy),
                                    _ptr(work), work.numel(), _stream(stream)))
+
+
+def chfsi_profile_enable(mesh, on: bool):
+    _check(lib().chfsi_profile_enable(mesh, int(bool(on))))
+
+
+def chfsi_profile_read(mesh):
+    """(cell-kernel ms summed, launches, algorithmic bytes summed) since the last read; synchronises."""
+    ms, n, by = C.c_double(), C.c_longlong(), C.c_double()
+    _check(lib().chfsi_profile_read(mesh, C.byref(ms), C.byref(n), C.byref(by)))
+    return ms.value, n.value, by.value
 
 
 def chfsi_last_launch_count() -> int:

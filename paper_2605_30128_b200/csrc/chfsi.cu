@@ -193,10 +193,36 @@ chfsi_status chfsi_mesh_create(int ncx, int ncy, int ncz, double Lx, double Ly, 
     return CHFSI_OK;
 }
 
+chfsi_status chfsi_profile_enable(chfsi_mesh* m, int on) {
+    if (!m) return fail(CHFSI_EINVAL, "profile_enable: mesh is NULL");
+    m->prof_on = on != 0;
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_profile_read(chfsi_mesh* m, double* cell_ms, long long* cell_launches, double* cell_alg_bytes) {
+    if (!m || !cell_ms || !cell_launches || !cell_alg_bytes) return fail(CHFSI_EINVAL, "profile_read: NULL argument");
+    DeviceGuard g(m->device);
+    double ms = 0.0;
+    for (size_t i = 0; i + 1 < m->prof_ev.size(); i += 2) {
+        CU(cudaEventSynchronize(m->prof_ev[i + 1]));
+        float t = 0.f;
+        CU(cudaEventElapsedTime(&t, m->prof_ev[i], m->prof_ev[i + 1]));
+        ms += t;
+    }
+    *cell_ms = ms;
+    *cell_launches = (long long)(m->prof_ev.size() / 2);
+    *cell_alg_bytes = m->prof_bytes;
+    for (cudaEvent_t e : m->prof_ev) cudaEventDestroy(e);
+    m->prof_ev.clear();
+    m->prof_bytes = 0.0;
+    return CHFSI_OK;
+}
+
 chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
     if (!m) return CHFSI_OK;
     {
         DeviceGuard g(m->device);
+        for (cudaEvent_t e : m->prof_ev) cudaEventDestroy(e);
         cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz);
         free_nonlocal(m->nl);
     }

@@ -107,6 +107,10 @@ struct chfsi_mesh {
     double* dBy = nullptr;
     double* dBz = nullptr;
     chfsi::NonlocalDev nl;
+    // profiling aid (chfsi_profile_enable / chfsi_profile_read)
+    mutable bool prof_on = false;
+    mutable std::vector<cudaEvent_t> prof_ev;      // start/stop pairs
+    mutable double prof_bytes = 0.0;
 };
 
 namespace chfsi {

@@ -359,8 +359,18 @@ static cudaError_t launch_cell_t(const chfsi_mesh* m, const CellArgs& a, cudaStr
     }
     const int nchunks = (a.nvec + NV - 1) / NV;
     const long long grid = (long long)m->mc.ncells * nchunks;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (m->prof_on) {
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return cudaGetLastError();
+        cudaEventRecord(e0, st);
+    }
     kern<<<(unsigned)grid, n * C, smem, st>>>(m->mc, a);
     count_launch();
+    if (m->prof_on) {
+        cudaEventRecord(e1, st);
+        m->prof_ev.push_back(e0); m->prof_ev.push_back(e1);
+        m->prof_bytes += 2.0 * (double)m->nnodes * a.nvec * (16.0 * (1 + (a.R != nullptr && a.cR != nullptr)) + 32.0);
+    }
     return cudaGetLastError();
 }
 
