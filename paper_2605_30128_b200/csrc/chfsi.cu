@@ -223,7 +223,7 @@ chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
     {
         DeviceGuard g(m->device);
         for (cudaEvent_t e : m->prof_ev) cudaEventDestroy(e);
-        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz);
+        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF);
         free_nonlocal(m->nl);
     }
     delete m;
@@ -299,6 +299,15 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
         else CU(cudaMemset(*dst[f], 0, M * sizeof(double)));
     }
     m->mc.V = m->dV; m->mc.Bx = m->dBx; m->mc.By = m->dBy; m->mc.Bz = m->dBz;
+    {   // packed copy for the march kernel: one 32-byte record per node
+        std::vector<double> F((size_t)M * 4);
+        for (long long I = 0; I < M; ++I) {
+            const double v = V ? V[I] : 0.0, bx = Bx ? Bx[I] : 0.0, by = By ? By[I] : 0.0, bz = Bz ? Bz[I] : 0.0;
+            F[4 * I + 0] = v + bz; F[4 * I + 1] = v - bz; F[4 * I + 2] = bx; F[4 * I + 3] = by;
+        }
+        if (m->dF == nullptr) CU(cudaMalloc(reinterpret_cast<void**>(&m->dF), (size_t)M * 32));
+        CU(cudaMemcpy(m->dF, F.data(), (size_t)M * 32, cudaMemcpyHostToDevice));
+    }
     // ---- nonlocal tables
     free_nonlocal(m->nl);
     NonlocalDev& nl = m->nl;

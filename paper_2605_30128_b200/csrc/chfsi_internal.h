@@ -106,6 +106,7 @@ struct chfsi_mesh {
     double* dBx = nullptr;
     double* dBy = nullptr;
     double* dBz = nullptr;
+    double* dF = nullptr;               // packed fields [M][4] = V+Bz, V-Bz, Bx, By (march kernel)
     chfsi::NonlocalDev nl;
     // profiling aid (chfsi_profile_enable / chfsi_profile_read)
     mutable bool prof_on = false;
@@ -130,6 +131,9 @@ struct CoefRow { double cin0, cinL, cinLam, cR0, cRL, al, be, ga, advance; };
 // table (device): row r = [cin(0..nvec-1), cR(0..nvec-1)]
 cudaError_t launch_coef(const double* hdr, double* table, int nrows, int nvec, cudaStream_t s);
 bool cell_supported(int p, chfsi_prec prec);
+// z-marching TMA kernel (cell_march.cu)
+bool march_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
+cudaError_t launch_cell_march(const chfsi_mesh* m, const CellArgs& a, cudaStream_t s);
 void set_error(const std::string& s);
 void count_launch(int n = 1);
 }  // namespace chfsi

@@ -1,6 +1,8 @@
 // sm_100a kernels of libchfsi: cell gather / sum-factorised Laplacian / fused pointwise update with
 // in-place L2 reductions (S1-S3, S5, S6 of DESIGN.md), nonlocal projector kernels (S4), and the
 // pointwise recover/scale kernel (S7).
+#include <cstdlib>
+
 #include "chfsi_internal.h"
 
 namespace chfsi {
@@ -359,18 +361,7 @@ static cudaError_t launch_cell_t(const chfsi_mesh* m, const CellArgs& a, cudaStr
     }
     const int nchunks = (a.nvec + NV - 1) / NV;
     const long long grid = (long long)m->mc.ncells * nchunks;
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (m->prof_on) {
-        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return cudaGetLastError();
-        cudaEventRecord(e0, st);
-    }
     kern<<<(unsigned)grid, n * C, smem, st>>>(m->mc, a);
-    count_launch();
-    if (m->prof_on) {
-        cudaEventRecord(e1, st);
-        m->prof_ev.push_back(e0); m->prof_ev.push_back(e1);
-        m->prof_bytes += 2.0 * (double)m->nnodes * a.nvec * (16.0 * (1 + (a.R != nullptr && a.cR != nullptr)) + 32.0);
-    }
     return cudaGetLastError();
 }
 
@@ -379,7 +370,35 @@ bool cell_supported(int p, chfsi_prec prec) {
     return p >= 1 && p <= 8;
 }
 
+static cudaError_t launch_cell_legacy(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t st);
+
+static bool use_legacy() {
+    static int v = -1;
+    if (v < 0) { const char* e = getenv("CHFSI_CELL_KERNEL"); v = (e && std::string(e) == "legacy") ? 1 : 0; }
+    return v == 1;
+}
+
+// The dominant kernel: the z-marching TMA kernel where it is instantiated (FP64; p = 2, 4, 6), else the
+// tile-per-cell kernel above (FP32 product; other degrees).  CHFSI_CELL_KERNEL=legacy forces the latter.
 cudaError_t launch_cell(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t st) {
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (m->prof_on) {
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return cudaGetLastError();
+        cudaEventRecord(e0, st);
+    }
+    cudaError_t err;
+    if (!use_legacy() && march_supported(m, prec, a)) err = launch_cell_march(m, a, st);
+    else err = launch_cell_legacy(m, prec, a, st);
+    count_launch();
+    if (m->prof_on) {
+        cudaEventRecord(e1, st);
+        m->prof_ev.push_back(e0); m->prof_ev.push_back(e1);
+        m->prof_bytes += 2.0 * (double)m->nnodes * a.nvec * (16.0 * (1 + (a.R != nullptr && a.cR != nullptr)) + 32.0);
+    }
+    return err;
+}
+
+static cudaError_t launch_cell_legacy(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t st) {
     const bool f32 = prec == CHFSI_FP32;
 #define CELL_CASE(PP, NV64, NV32)                                                     \
     case PP:                                                                           \
