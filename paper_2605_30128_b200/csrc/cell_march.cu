@@ -91,7 +91,7 @@ struct MarchCfg {
 };
 
 // Per-thread state of a consumer warp (row j of the footprint, lane = batch column).
-template <int P>
+template <int P, bool HASPH>
 struct MarchConsumer {
     using Cfg = MarchCfg<P>;
     static constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES;
@@ -100,7 +100,7 @@ struct MarchConsumer {
     double wyj, pyj, fyj, cin, cR;
     double* outcol;
     int j, col, s_spin, ri, ex, gy, g0;
-    bool vok, hasph, jown, wy, xwrap, ywrap;
+    bool vok, jown, wy, xwrap, ywrap;
 
     __device__ __forceinline__ void init(const StepConst& sc, const MarchArgs& ar, int warp, int lane, int ex_, int ey,
                                          int chunk, int g0_, bool xw, bool yw) {
@@ -109,7 +109,6 @@ struct MarchConsumer {
         const int vl = (col & 15) >> 1;
         const int v = chunk * 8 + vl;
         vok = v < ar.nvec;
-        hasph = ar.has_phase != 0;
         jown = j < P;
 #pragma unroll
         for (int b = 0; b < n; ++b) { kyrow[b] = sc.KY[j][b]; wxy[b] = sc.WX[b] * sc.WY[j]; }
@@ -124,57 +123,61 @@ struct MarchConsumer {
             for (int a = 0; a < n; ++a) acc[k][a] = 0.0;
     }
 
+    __device__ __forceinline__ static void phase_of(const MarchArgs& ar, bool wx, bool wyy, bool wz, double& pr, double& pi) {
+        pr = 1.0; pi = 0.0;
+        if (wx) { pr = ar.ph_re[0]; pi = ar.ph_im[0]; }
+        if (wyy) { const double tt = pr * ar.ph_re[1] - pi * ar.ph_im[1]; pi = pr * ar.ph_im[1] + pi * ar.ph_re[1]; pr = tt; }
+        if (wz) { const double tt = pr * ar.ph_re[2] - pi * ar.ph_im[2]; pi = pr * ar.ph_im[2] + pi * ar.ph_re[2]; pr = tt; }
+    }
+
     // emit planes [0, nk) of the accumulators to global planes gzbase + k  (S3: one RED.ADD.F64 per node and column)
     __device__ __forceinline__ void emit(const MarchArgs& ar, int gzbase, int nk) {
+        const long long xstride = 4 * ar.ld_out;                       // doubles between consecutive nodes
+        const long long x0 = (long long)ex * P;
 #pragma unroll
         for (int k = 0; k < n; ++k) {
             if (k < nk) {
                 int gz = gzbase + k; const bool wz = gz == ar.n1[2]; if (wz) gz = 0;
-                const long long line0 = ((long long)gz * ar.n1[1] + gy) * ar.n1[0];
+                double* line = outcol + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xstride;
+                double* pnode = line + x0 * xstride;
 #pragma unroll
                 for (int a = 0; a < n; ++a) {
-                    int gx = ex * P + a; const bool wx = gx == ar.n1[0]; if (wx) gx = 0;
+                    const bool wx = (a == P) && xwrap;
+                    double* dst = wx ? line : pnode + a * xstride;
                     double val = acc[k][a];
-                    if (hasph) {
+                    if (HASPH) {
                         const double other = __shfl_xor_sync(0xffffffffu, val, 1);
                         if (wx | wy | wz) {
-                            double pr = 1.0, pi = 0.0;
-                            if (wx) { pr = ar.ph_re[0]; pi = ar.ph_im[0]; }
-                            if (wy) { const double tt = pr * ar.ph_re[1] - pi * ar.ph_im[1]; pi = pr * ar.ph_im[1] + pi * ar.ph_re[1]; pr = tt; }
-                            if (wz) { const double tt = pr * ar.ph_re[2] - pi * ar.ph_im[2]; pi = pr * ar.ph_im[2] + pi * ar.ph_re[2]; pr = tt; }
+                            double pr, pi; phase_of(ar, wx, wy, wz, pr, pi);
                             val = ri == 0 ? val * pr + other * pi : val * pr - other * pi;   // times conj(phase)
                         }
                     }
-                    if (vok) atomicAdd(outcol + (line0 + gx) * 4 * ar.ld_out, val);
+                    if (vok) atomicAdd(dst, val);
                 }
             }
         }
     }
 
-    // One plane; CL = its local index in the current cell (upper role).  lower: it is also plane P of the previous
-    // cell; upper: it belongs to a cell of this segment (false only for the segment's last plane).
-    template <int CL>
+    // One plane t of the march.  c = its local index in the current cell (upper role); lower: it is also plane P of
+    // the previous cell; upper: it belongs to a cell of this segment (false only for the segment's last plane).
     __device__ __forceinline__ void plane(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, uint64_t* full_bar,
-                                          uint64_t* empty_bar, int t, bool lower, bool upper) {
+                                          uint64_t* empty_bar, int t, int c, bool lower, bool upper) {
         const int s = t % STAGES;
         const uint32_t par = (t / STAGES) & 1;
         mbar_wait(&full_bar[s], par);
         double* IN = reinterpret_cast<double*>(smem + (size_t)s * Cfg::STAGE_BYTES);
         const double* Rs = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES + Cfg::R_OFF);
         const double* Fs = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES + Cfg::F_OFF);
-        if (hasph) {
+        if (HASPH) {
             // Bloch phase on wrapped entries (x: column a = P; y: row j = P; z: the wrapped plane), fixed up in place
             const bool wz = (g0 + t) == ar.n1[2];
             if (xwrap | ywrap | wz) {
-#pragma unroll
+                const bool wyy = ywrap && j == P;
+#pragma unroll 1
                 for (int a = 0; a < n; ++a) {
                     const bool wx = xwrap && a == P;
-                    const bool wyy = ywrap && j == P;
                     if (wx | wyy | wz) {
-                        double pr = 1.0, pi = 0.0;
-                        if (wx) { pr = ar.ph_re[0]; pi = ar.ph_im[0]; }
-                        if (wyy) { const double tt = pr * ar.ph_re[1] - pi * ar.ph_im[1]; pi = pr * ar.ph_im[1] + pi * ar.ph_re[1]; pr = tt; }
-                        if (wz) { const double tt = pr * ar.ph_re[2] - pi * ar.ph_im[2]; pi = pr * ar.ph_im[2] + pi * ar.ph_re[2]; pr = tt; }
+                        double pr, pi; phase_of(ar, wx, wyy, wz, pr, pi);
                         const double val = IN[(j * n + a) * C + col];
                         const double other = __shfl_xor_sync(0xffffffffu, val, 1);
                         IN[(j * n + a) * C + col] = ri == 0 ? val * pr - other * pi : other * pi + val * pr;
@@ -183,25 +186,26 @@ struct MarchConsumer {
                 asm volatile("bar.sync 1, %0;" ::"r"(n * 32) : "memory");   // consumer warps only
             }
         }
+        const double* INc = IN + col;
         double row[n];
 #pragma unroll
-        for (int a = 0; a < n; ++a) row[a] = IN[(j * n + a) * C + col];
+        for (int a = 0; a < n; ++a) row[a] = INc[(j * n + a) * C];
         double ip[n];
+        // y-contraction: column a of the plane against row j of KY
+#pragma unroll
+        for (int a = 0; a < n; ++a) {
+            double sy = 0.0;
+#pragma unroll
+            for (int b = 0; b < n; ++b) sy = fma(kyrow[b], INc[(b * n + a) * C], sy);
+            ip[a] = sc.WX[a] * sy;
+        }
         // x-contraction on the own row
 #pragma unroll
         for (int i = 0; i < n; ++i) {
             double sx = 0.0;
 #pragma unroll
             for (int a = 0; a < n; ++a) sx = fma(sc.KX[i][a], row[a], sx);
-            ip[i] = wyj * sx;
-        }
-        // y-contraction: column a of the plane against row j of KY
-#pragma unroll
-        for (int a = 0; a < n; ++a) {
-            double sy = 0.0;
-#pragma unroll
-            for (int b = 0; b < n; ++b) sy = fma(kyrow[b], IN[(b * n + a) * C + col], sy);
-            ip[a] = fma(sc.WX[a], sy, ip[a]);
+            ip[i] = fma(wyj, sx, ip[i]);
         }
         double zr[n];
 #pragma unroll
@@ -223,30 +227,42 @@ struct MarchConsumer {
                 for (int a = 0; a < n; ++a) acc[k][a] = 0.0;
         }
         if (upper) {
+            // z-push with the runtime cell-local index c: column c of KZ fetched from the constant bank
 #pragma unroll
-            for (int k = 0; k < n; ++k)
+            for (int k = 0; k < n; ++k) {
+                const double kz = sc.KZ[k][c];
 #pragma unroll
-                for (int a = 0; a < n; ++a) acc[k][a] = fma(sc.KZ[k][CL], zr[a], acc[k][a]);
+                for (int a = 0; a < n; ++a) acc[k][a] = fma(kz, zr[a], acc[k][a]);
+            }
+            const double wzc = sc.WZ[c];
 #pragma unroll
-            for (int a = 0; a < n; ++a) acc[CL][a] = fma(sc.WZ[CL], ip[a], acc[CL][a]);
+            for (int a = 0; a < n; ++a) ip[a] *= wzc;
             if (jown) {
                 // S5 on the owned nodes of this plane (a < P): eq. 12 spin blocks, in-term, R-term
-                const double pz = sc.PZ[CL] * pyj, fz = sc.FZ[CL] * fyj;
+                const double pz = sc.PZ[c] * pyj, fz = sc.FZ[c] * fyj * cin;
 #pragma unroll
                 for (int a = 0; a < P; ++a) {
                     const double in_own = row[a];
-                    const double o_same = IN[(j * n + a) * C + (col ^ 16)];
-                    const double o_flip = IN[(j * n + a) * C + (col ^ 17)];
+                    const double o_same = INc[(j * n + a) * C + ((col ^ 16) - col)];
+                    const double o_flip = INc[(j * n + a) * C + ((col ^ 17) - col)];
                     const double u_re = ri == 0 ? o_same : o_flip;       // other spin, same vector
                     const double u_im = ri == 0 ? o_flip : o_same;
                     const double4 f = *reinterpret_cast<const double4*>(Fs + (j * P + a) * 4);
                     const double diag = s_spin == 0 ? f.x : f.y;
                     const double sy = s_spin == 0 ? -f.w : f.w;
                     const double offd = ri == 0 ? f.z * u_re - sy * u_im : f.z * u_im + sy * u_re;
-                    double val = (pz * sc.PX[a]) * (diag * in_own + offd);
-                    val = fma(cin * (fz * sc.FX[a]), in_own, val);
+                    double val = fma(pz * sc.PX[a], fma(diag, in_own, offd), ip[a]);
+                    val = fma(fz * sc.FX[a], in_own, val);
                     if (ar.useR) val = fma(cR, Rs[(j * P + a) * C + col], val);
-                    acc[CL][a] += val;
+                    ip[a] = val;
+                }
+            }
+            // add the in-plane + pointwise part to the accumulator of the plane's own index
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                if (c == k) {
+#pragma unroll
+                    for (int a = 0; a < n; ++a) acc[k][a] += ip[a];
                 }
             }
         }
@@ -255,7 +271,7 @@ struct MarchConsumer {
     }
 };
 
-template <int P>
+template <int P, bool HASPH>
 __global__ void __launch_bounds__(MarchCfg<P>::THREADS, 1)
 cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ MarchArgs ar,
                   const __grid_constant__ CUtensorMap map_in_full, const __grid_constant__ CUtensorMap map_in_p,
@@ -318,21 +334,15 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
     }
 
     // ================================ consumers ================================
-    MarchConsumer<P> cs;
+    MarchConsumer<P, HASPH> cs;
     cs.init(sc, ar, warp, lane, ex, ey, chunk, g0, xwrap, ywrap);
-    int t = 0;
-    for (int cell = 0; cell < ar.cps; ++cell) {
-        cs.template plane<0>(sc, ar, smem, full_bar, empty_bar, t, cell > 0, true); ++t;
-        if constexpr (P > 1) { cs.template plane<1 % n>(sc, ar, smem, full_bar, empty_bar, t, false, true); ++t; }
-        if constexpr (P > 2) { cs.template plane<2 % n>(sc, ar, smem, full_bar, empty_bar, t, false, true); ++t; }
-        if constexpr (P > 3) { cs.template plane<3 % n>(sc, ar, smem, full_bar, empty_bar, t, false, true); ++t; }
-        if constexpr (P > 4) { cs.template plane<4 % n>(sc, ar, smem, full_bar, empty_bar, t, false, true); ++t; }
-        if constexpr (P > 5) { cs.template plane<5 % n>(sc, ar, smem, full_bar, empty_bar, t, false, true); ++t; }
-        if constexpr (P > 6) { cs.template plane<6 % n>(sc, ar, smem, full_bar, empty_bar, t, false, true); ++t; }
-        if constexpr (P > 7) { cs.template plane<7 % n>(sc, ar, smem, full_bar, empty_bar, t, false, true); ++t; }
+    int c = 0;
+#pragma unroll 1
+    for (int t = 0; t < T; ++t) {
+        cs.plane(sc, ar, smem, full_bar, empty_bar, t, c, c == 0 && t > 0, t < T - 1);
+        c = (c + 1 == P) ? 0 : c + 1;
     }
-    cs.template plane<0>(sc, ar, smem, full_bar, empty_bar, t, true, false);   // last plane: lower role only
-    cs.emit(ar, g0 + t, 1);                                                    // its partial (top face of the segment)
+    cs.emit(ar, g0 + T - 1, 1);                                   // partial of the segment's top face
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -427,12 +437,13 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
         !make_map(&mr, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, rows, 2 * P))
         return cudaErrorInvalidValue;
     const size_t smem = (size_t)Cfg::STAGES * Cfg::STAGE_BYTES;
-    static bool attr_done[64] = {false};
-    auto kern = cell_march_kernel<P>;
-    if (!attr_done[m->device & 63]) {
+    static bool attr_done[128] = {false};
+    auto kern = m->mc.has_phase ? cell_march_kernel<P, true> : cell_march_kernel<P, false>;
+    const int slot = (m->device & 63) * 2 + (m->mc.has_phase ? 1 : 0);
+    if (!attr_done[slot]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_done[m->device & 63] = true;
+        attr_done[slot] = true;
     }
     const long long grid = base * nseg;
     kern<<<(unsigned)grid, Cfg::THREADS, smem, st>>>(sc, ar, mf, mp, m1, mr);
