@@ -116,7 +116,7 @@ static WorkLayout work_layout(const chfsi_mesh* m, chfsi_recur recur, int chunk,
     wl.nbuf = recur == CHFSI_RECUR_RESIDUAL ? 3 : 1;
     wl.hdr_bytes = align256((size_t)(4 + 9 * (degree_cap + 2) + chunk) * sizeof(double));
     wl.coef_bytes = align256((size_t)(degree_cap + 2) * 2 * chunk * sizeof(double));
-    wl.c_bytes = align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * chunk * 16);
+    wl.c_bytes = 2 * align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * chunk * 16);   // C and G
     wl.buf_bytes = align256((size_t)2 * m->nnodes * chunk * 16);
     wl.total = wl.hdr_bytes + wl.coef_bytes + wl.c_bytes + wl.nbuf * wl.buf_bytes;
     return wl;
@@ -314,7 +314,7 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
     nl.natoms = natoms; nl.nnz = nnz; nl.max_nproj = max_np; nl.crows = crows;
     if (natoms > 0 && nnz > 0) {
         std::vector<ProjItem> items;
-        constexpr int kSlice = 64;
+        constexpr int kSlice = 8;    // must match kernels.cu
         for (int a = 0; a < natoms; ++a) {
             const long long ns = supp_off[a + 1] - supp_off[a];
             for (long long st = 0; st < ns; st += kSlice)
@@ -371,7 +371,9 @@ static chfsi_status accumulate_H(const chfsi_mesh* m, chfsi_prec prec, const Cel
     }
     CU(launch_cell(m, prec, ca, st));
     if (nlocal) {
-        BackArgs ba{Cbuf, ca.out, ca.ld_out, ca.cH, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
+        double* Gbuf = reinterpret_cast<double*>(reinterpret_cast<char*>(Cbuf) +
+                                                 align256((size_t)m->nl.crows * ca.nvec * 16));
+        BackArgs ba{Cbuf, Gbuf, ca.out, ca.ld_out, ca.cH, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
         CU(launch_back(m, prec, ba, st));
     }
     return CHFSI_OK;
@@ -396,7 +398,7 @@ chfsi_status chfsi_apply_H(const chfsi_mesh* m, chfsi_prec prec, int nvec, const
     chfsi_status stt = check_common(m, prec, nvec, X, ldx, Y, ldy, work, "apply_H");
     if (stt != CHFSI_OK) return stt;
     if (X == Y) return fail(CHFSI_EINVAL, "apply_H: X and Y must be distinct");
-    const size_t need = align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * nvec * 16);
+    const size_t need = 2 * align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * nvec * 16);
     if (work_bytes < need) return fail(CHFSI_EINVAL, "apply_H: work_bytes too small");
     DeviceGuard g(m->device);
     if (!g.ok) return fail(CHFSI_ECUDA, "apply_H: cannot select device");

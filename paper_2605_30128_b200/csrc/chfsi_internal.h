@@ -83,6 +83,7 @@ struct ProjArgs {
 
 struct BackArgs {
     const double* C;                    // projected coefficients
+    double* G;                          // scratch for G = D C, same shape as C
     double* out; long long ld_out;
     double cH;
     int nvec;

@@ -197,8 +197,14 @@ cell_kernel(const __grid_constant__ MeshConst mc, const __grid_constant__ CellAr
 }
 
 // ---------------------------------------------------------------------------------------------
-// S4 forward projection: C_a[2 beta + s][v] += sum_{I in slice} conj(P_a[I,beta]) u_{I,s,v}
-// One CTA = one slice of an atom's support x 128 (spin, vector) columns.
+// S4 nonlocal term (PAPER.md:204 stage (iv)): three small kernels per H application.
+//   proj : C_a[2 beta + s][v] += sum_{I in slice} conj(P_a[I,beta]) u_{I,s,v}      (skinny GEMM, RED into C)
+//   gmat : G_a = D_a C_a                                                            ((2 nproj)^2 per atom)
+//   back : out_{I,s,v} += cH * f_I * sum_beta P_a[I,beta] G_a[2 beta + s][v]        (RED into out)
+// A slice is kSlice support nodes, fully unrolled so that all its loads are in flight at once; one CTA =
+// one slice x 128 (spin, vector) columns.
+constexpr int kSlice = 8;
+
 template <typename TT>
 __global__ void __launch_bounds__(128)
 proj_kernel(const NonlocalDev nl, const ProjArgs ar) {
@@ -207,41 +213,59 @@ proj_kernel(const NonlocalDev nl, const ProjArgs ar) {
     const int v = (blockIdx.y >> 1) * 128 + threadIdx.x;
     if (v >= ar.nvec) return;
     const int np = nl.nproj[it.atom];
-    const long long soff = nl.s_off[it.atom];
-    const long long poff = nl.p_off[it.atom];
-    TT acc_re[kMaxProj], acc_im[kMaxProj];
+    const long long soff = nl.s_off[it.atom] + it.start;
+    const long long poff = nl.p_off[it.atom] + (long long)it.start * np;
+    double2 x[kSlice];
 #pragma unroll
-    for (int b = 0; b < kMaxProj; ++b) { acc_re[b] = 0; acc_im[b] = 0; }
-    for (int jj = 0; jj < it.count; ++jj) {
-        const long long j = it.start + jj;                 // index within the atom's support
-        const long long I = nl.supp_node[soff + j];
-        double2 x = __ldg(reinterpret_cast<const double2*>(ar.in) + (2 * I + s) * ar.ld_in + v);
-        if (ar.mass_u) { const double m = nl.supp_mass[soff + j]; x.x *= m; x.y *= m; }
-        const TT xr = (TT)x.x, xi = (TT)x.y;
-#pragma unroll
-        for (int b = 0; b < kMaxProj; ++b) {
-            if (b < np) {
-                TT pr, pi;
-                if (sizeof(TT) == 8) { const double2 pv = nl.P64[poff + j * np + b]; pr = pv.x; pi = pv.y; }
-                else { const float2 pv = nl.P32[poff + j * np + b]; pr = pv.x; pi = pv.y; }
-                // conj(p) x = (pr - i pi)(xr + i xi)
-                acc_re[b] = fma(pr, xr, fma(pi, xi, acc_re[b]));
-                acc_im[b] = fma(pr, xi, fma(-pi, xr, acc_im[b]));
-            }
+    for (int jj = 0; jj < kSlice; ++jj) {
+        x[jj] = make_double2(0.0, 0.0);
+        if (jj < it.count) {
+            const long long I = nl.supp_node[soff + jj];
+            x[jj] = __ldg(reinterpret_cast<const double2*>(ar.in) + (2 * I + s) * ar.ld_in + v);
+            if (ar.mass_u) { const double m = nl.supp_mass[soff + jj]; x[jj].x *= m; x[jj].y *= m; }
         }
     }
     double* Crow = ar.C + (nl.c_off[it.atom] * (long long)ar.nvec + v) * 2;
+    for (int b = 0; b < np; ++b) {
+        TT cr = 0, ci = 0;
 #pragma unroll
-    for (int b = 0; b < kMaxProj; ++b) {
-        if (b < np) {
-            double* dst = Crow + (long long)(2 * b + s) * ar.nvec * 2;
-            red_add(dst, (double)acc_re[b]);
-            red_add(dst + 1, (double)acc_im[b]);
+        for (int jj = 0; jj < kSlice; ++jj) {
+            if (jj < it.count) {
+                TT pr, pi;
+                if (sizeof(TT) == 8) { const double2 pv = nl.P64[poff + jj * np + b]; pr = pv.x; pi = pv.y; }
+                else { const float2 pv = nl.P32[poff + jj * np + b]; pr = pv.x; pi = pv.y; }
+                const TT xr = (TT)x[jj].x, xi = (TT)x[jj].y;
+                cr = fma(pr, xr, fma(pi, xi, cr));                   // conj(p) x = (pr - i pi)(xr + i xi)
+                ci = fma(pr, xi, fma(-pi, xr, ci));
+            }
         }
+        double* dst = Crow + (long long)(2 * b + s) * ar.nvec * 2;
+        red_add(dst, (double)cr);
+        red_add(dst + 1, (double)ci);
     }
 }
 
-// S4 back projection: out_{I,s,v} += cH * f_I * sum_beta P_a[I,beta] G_a[2 beta + s][v],  G_a = D_a C_a
+// G[c_off + row][v] = sum_r D_a[row][r] C[c_off + r][v]; one thread per (row, v)
+__global__ void __launch_bounds__(128)
+gmat_kernel(const NonlocalDev nl, const double2* __restrict__ Cc, double2* __restrict__ G, int nvec) {
+    const int atom = blockIdx.x;
+    const int np2 = 2 * nl.nproj[atom];
+    const int row = blockIdx.y;
+    const int v = blockIdx.z * 128 + threadIdx.x;
+    if (row >= np2 || v >= nvec) return;
+    const double2* D = nl.D64 + nl.d_off[atom] + (long long)row * np2;
+    const double2* c = Cc + nl.c_off[atom] * (long long)nvec + v;
+    double gr = 0.0, gi = 0.0;
+#pragma unroll 8
+    for (int r = 0; r < np2; ++r) {
+        const double2 d = D[r];
+        const double2 cv = c[(long long)r * nvec];
+        gr += d.x * cv.x - d.y * cv.y;
+        gi += d.x * cv.y + d.y * cv.x;
+    }
+    G[(nl.c_off[atom] + row) * (long long)nvec + v] = make_double2(gr, gi);
+}
+
 template <typename TT>
 __global__ void __launch_bounds__(128)
 back_kernel(const NonlocalDev nl, const BackArgs ar) {
@@ -250,43 +274,35 @@ back_kernel(const NonlocalDev nl, const BackArgs ar) {
     const int v = (blockIdx.y >> 1) * 128 + threadIdx.x;
     if (v >= ar.nvec) return;
     const int np = nl.nproj[it.atom];
-    const long long soff = nl.s_off[it.atom];
-    const long long poff = nl.p_off[it.atom];
-    const double2* D = nl.D64 + nl.d_off[it.atom];
-    const double2* Cc = reinterpret_cast<const double2*>(ar.C) + nl.c_off[it.atom] * (long long)ar.nvec + v;
-    TT g_re[kMaxProj], g_im[kMaxProj];
+    const long long soff = nl.s_off[it.atom] + it.start;
+    const long long poff = nl.p_off[it.atom] + (long long)it.start * np;
+    const double2* G = reinterpret_cast<const double2*>(ar.G) + nl.c_off[it.atom] * (long long)ar.nvec + v;
+    TT yr[kSlice], yi[kSlice];
 #pragma unroll
-    for (int b = 0; b < kMaxProj; ++b) {
-        double gr = 0.0, gi = 0.0;
-        if (b < np) {
-            const int row = 2 * b + s;
-            for (int r = 0; r < 2 * np; ++r) {
-                const double2 d = D[row * 2 * np + r];
-                const double2 c = Cc[(long long)r * ar.nvec];
-                gr += d.x * c.x - d.y * c.y;
-                gi += d.x * c.y + d.y * c.x;
-            }
-        }
-        g_re[b] = (TT)gr; g_im[b] = (TT)gi;
-    }
-    for (int jj = 0; jj < it.count; ++jj) {
-        const long long j = it.start + jj;
-        const long long I = nl.supp_node[soff + j];
-        TT yr = 0, yi = 0;
+    for (int jj = 0; jj < kSlice; ++jj) { yr[jj] = 0; yi[jj] = 0; }
+    for (int b = 0; b < np; ++b) {
+        const double2 g = G[(long long)(2 * b + s) * ar.nvec];
+        const TT gr = (TT)g.x, gi = (TT)g.y;
 #pragma unroll
-        for (int b = 0; b < kMaxProj; ++b) {
-            if (b < np) {
+        for (int jj = 0; jj < kSlice; ++jj) {
+            if (jj < it.count) {
                 TT pr, pi;
-                if (sizeof(TT) == 8) { const double2 pv = nl.P64[poff + j * np + b]; pr = pv.x; pi = pv.y; }
-                else { const float2 pv = nl.P32[poff + j * np + b]; pr = pv.x; pi = pv.y; }
-                yr = fma(pr, g_re[b], fma(-pi, g_im[b], yr));
-                yi = fma(pr, g_im[b], fma(pi, g_re[b], yi));
+                if (sizeof(TT) == 8) { const double2 pv = nl.P64[poff + jj * np + b]; pr = pv.x; pi = pv.y; }
+                else { const float2 pv = nl.P32[poff + jj * np + b]; pr = pv.x; pi = pv.y; }
+                yr[jj] = fma(pr, gr, fma(-pi, gi, yr[jj]));
+                yi[jj] = fma(pr, gi, fma(pi, gr, yi[jj]));
             }
         }
-        const double f = ar.cH * (ar.sout_invm ? 1.0 : nl.supp_mass[soff + j]);
-        double* dst = ar.out + ((2 * I + s) * ar.ld_out + v) * 2;
-        red_add(dst, f * (double)yr);
-        red_add(dst + 1, f * (double)yi);
+    }
+#pragma unroll
+    for (int jj = 0; jj < kSlice; ++jj) {
+        if (jj < it.count) {
+            const long long I = nl.supp_node[soff + jj];
+            const double f = ar.cH * (ar.sout_invm ? 1.0 : nl.supp_mass[soff + jj]);
+            double* dst = ar.out + ((2 * I + s) * ar.ld_out + v) * 2;
+            red_add(dst, f * (double)yr[jj]);
+            red_add(dst + 1, f * (double)yi[jj]);
+        }
     }
 }
 
@@ -428,6 +444,12 @@ cudaError_t launch_proj(const chfsi_mesh* m, chfsi_prec prec, const ProjArgs& a,
 
 cudaError_t launch_back(const chfsi_mesh* m, chfsi_prec prec, const BackArgs& a, cudaStream_t st) {
     if (m->nl.nitems == 0) return cudaSuccess;
+    {
+        dim3 gg(m->nl.natoms, 2 * m->nl.max_nproj, (a.nvec + 127) / 128);
+        gmat_kernel<<<gg, 128, 0, st>>>(m->nl, reinterpret_cast<const double2*>(a.C),
+                                        reinterpret_cast<double2*>(a.G), a.nvec);
+        count_launch();
+    }
     dim3 grid(m->nl.nitems, 2 * ((a.nvec + 127) / 128));
     if (prec == CHFSI_FP32) back_kernel<float><<<grid, 128, 0, st>>>(m->nl, a);
     else back_kernel<double><<<grid, 128, 0, st>>>(m->nl, a);
