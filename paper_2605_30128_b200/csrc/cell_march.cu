@@ -49,6 +49,14 @@ struct MarchArgs {
     long long ld_out;
 };
 
+// Tensor maps of one launch.  main/face[0]: n lines, [1]: P lines, [2]: 1 line (the y-wrapped line of the last cell row).
+struct MarchMaps {
+    CUtensorMap main[3];    // box (C/2 doubles, 2P rows, lines) of `in`
+    CUtensorMap face[3];    // box (C/2 doubles, 2 rows, lines) of `in`: the x = P column
+    CUtensorMap R;          // box (C/2 doubles, 2P rows, P lines) of R
+    CUtensorMap F;          // box (4P doubles, P lines) of the packed fields
+};
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count));
@@ -71,56 +79,79 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-template <int P>
+// Thread mapping of the consumers.  A consumer thread is (x-part h, footprint row j, batch column col):
+//   warp w -> h = w / WPH;  j = (w % WPH) * RPW + lane / C;  col = lane % C.
+// Part h owns the x-positions [h*NA, min(n, (h+1)*NA)) of its row: it computes the x-, y- and z-contractions
+// only for those outputs, so the (p+1) z-accumulator planes cost NA (not p+1) registers each and the CTA runs
+// XS times as many warps.  Rows are padded to whole warps (RPW = 32 / C rows per warp), so a warp never mixes parts.
+template <int P, int CC, int XSPLIT>
 struct MarchCfg {
     static constexpr int n = P + 1;
-    static constexpr int C = 32;                          // real batch columns per CTA (NV = 8 complex)
+    static constexpr int C = CC;                          // real batch columns per CTA (NV = C / 4 complex vectors)
+    static constexpr int NV = C / 4;
+    static constexpr int XS = XSPLIT;
+    static constexpr int NA = (n + XS - 1) / XS;
+    static constexpr int RPW = 32 / C;
+    static constexpr int WPH = (n + RPW - 1) / RPW;
+    static constexpr int CWARPS = XS * WPH;
+    static constexpr int THREADS = (CWARPS + 1) * 32;
+    // stage layout: MAIN [n lines][P nodes][C] | FACE [n lines][C] (the x = P column) | R [P][P][C] | fields [P][P][4]
+    static constexpr int FACE_OFF = n * P * C * 8;
     static constexpr int IN_BYTES = n * n * C * 8;
+    __host__ __device__ static constexpr int ofs(int b, int a) { return a < P ? (b * P + a) * C : (n * P + b) * C; }   // doubles
     static constexpr int R_BYTES = P * P * C * 8;
     static constexpr int F_BYTES = P * P * 32;
     static constexpr int R_OFF = IN_BYTES;
     static constexpr int F_OFF = IN_BYTES + R_BYTES;
     static constexpr int STAGE_BYTES = ((F_OFF + F_BYTES + 127) / 128) * 128;
     static constexpr int STAGES = (200 * 1024 / STAGE_BYTES) < 8 ? (200 * 1024 / STAGE_BYTES) : 8;
-    static constexpr int THREADS = (n + 1) * 32;
 };
 
-// Per-thread state of a consumer warp (row j of the footprint, lane = batch column).
-template <int P, bool HASPH>
+// Per-thread state of a consumer (part H of row j, lane = batch column).
+template <int P, int CC, int XSPLIT, bool HASPH, int H>
 struct MarchConsumer {
-    using Cfg = MarchCfg<P>;
+    using Cfg = MarchCfg<P, CC, XSPLIT>;
     static constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES;
-    double acc[n][n];            // z-accumulators of the current cell: acc[k][a], plane k, x-position a
-    double kyrow[n], wxy[n];
+    static constexpr int A0 = H * Cfg::NA;
+    static constexpr int NAH = (n - A0) < Cfg::NA ? (n - A0) : Cfg::NA;
+    double acc[n][NAH];          // z-accumulators of the current cell: acc[k][ii], plane k, x-position A0 + ii
+    double kyrow[n], wxy[NAH];
     double wyj, pyj, fyj, cin, cR;
     double* outcol;
     int j, col, s_spin, ri, ex, gy, g0;
-    bool vok, jown, wy, xwrap, ywrap;
+    bool vok, jown, wy, xwrap, ywrap, valid;
 
-    __device__ __forceinline__ void init(const StepConst& sc, const MarchArgs& ar, int warp, int lane, int ex_, int ey,
+    __device__ __forceinline__ void init(const StepConst& sc, const MarchArgs& ar, int row, int col_, int ex_, int ey,
                                          int chunk, int g0_, bool xw, bool yw) {
-        j = warp; col = lane; ex = ex_; g0 = g0_; xwrap = xw; ywrap = yw;
-        s_spin = col >> 4; ri = col & 1;
-        const int vl = (col & 15) >> 1;
-        const int v = chunk * 8 + vl;
-        vok = v < ar.nvec;
+        valid = row < n;
+        j = valid ? row : n - 1; col = col_; ex = ex_; g0 = g0_; xwrap = xw; ywrap = yw;
+        s_spin = col / (C / 2); ri = col & 1;
+        const int vl = (col % (C / 2)) >> 1;
+        const int v = chunk * Cfg::NV + vl;
+        vok = valid && v < ar.nvec;
         jown = j < P;
 #pragma unroll
-        for (int b = 0; b < n; ++b) { kyrow[b] = sc.KY[j][b]; wxy[b] = sc.WX[b] * sc.WY[j]; }
+        for (int b = 0; b < n; ++b) kyrow[b] = sc.KY[j][b];
+#pragma unroll
+        for (int ii = 0; ii < NAH; ++ii) wxy[ii] = sc.WX[A0 + ii] * sc.WY[j];
         wyj = sc.WY[j]; pyj = sc.PY[j]; fyj = sc.FY[j];
         cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
         cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
         gy = ey * P + j; wy = gy == ar.n1[1]; if (wy) gy = 0;
-        outcol = ar.out + ((long long)s_spin * ar.ld_out + v) * 2 + ri;
+        outcol = ar.out + ((long long)s_spin * ar.ld_out + (vok ? v : 0)) * 2 + ri;
 #pragma unroll
         for (int k = 0; k < n; ++k)
 #pragma unroll
-            for (int a = 0; a < n; ++a) acc[k][a] = 0.0;
+            for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = 0.0;
     }
 
     __device__ __forceinline__ static void phase_of(const MarchArgs& ar, bool wx, bool wyy, bool wz, double& pr, double& pi) {
@@ -130,10 +161,12 @@ struct MarchConsumer {
         if (wz) { const double tt = pr * ar.ph_re[2] - pi * ar.ph_im[2]; pi = pr * ar.ph_im[2] + pi * ar.ph_re[2]; pr = tt; }
     }
 
-    // emit planes [0, nk) of the accumulators to global planes gzbase + k  (S3: one RED.ADD.F64 per node and column)
+    // emit planes [0, nk) of the accumulators to global planes gzbase + k  (S3: one RED.ADD.F64 per node and column).
+    // The REDs are left individually predicated on purpose: ptxas then spreads them between the FMAs of the
+    // surrounding z-push; hoisting the predicate into one branch bunches 6(p+1) REDs together and costs 15 %.
     __device__ __forceinline__ void emit(const MarchArgs& ar, int gzbase, int nk) {
         const long long xstride = 4 * ar.ld_out;                       // doubles between consecutive nodes
-        const long long x0 = (long long)ex * P;
+        const long long x0 = (long long)ex * P + A0;
 #pragma unroll
         for (int k = 0; k < n; ++k) {
             if (k < nk) {
@@ -141,10 +174,10 @@ struct MarchConsumer {
                 double* line = outcol + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xstride;
                 double* pnode = line + x0 * xstride;
 #pragma unroll
-                for (int a = 0; a < n; ++a) {
-                    const bool wx = (a == P) && xwrap;
-                    double* dst = wx ? line : pnode + a * xstride;
-                    double val = acc[k][a];
+                for (int ii = 0; ii < NAH; ++ii) {
+                    const bool wx = (A0 + ii == P) && xwrap;
+                    double* dst = wx ? line : pnode + ii * xstride;
+                    double val = acc[k][ii];
                     if (HASPH) {
                         const double other = __shfl_xor_sync(0xffffffffu, val, 1);
                         if (wx | wy | wz) {
@@ -169,62 +202,63 @@ struct MarchConsumer {
         const double* Rs = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES + Cfg::R_OFF);
         const double* Fs = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES + Cfg::F_OFF);
         if (HASPH) {
-            // Bloch phase on wrapped entries (x: column a = P; y: row j = P; z: the wrapped plane), fixed up in place
+            // Bloch phase on wrapped entries (x: column a = P; y: row j = P; z: the wrapped plane), fixed up in place;
+            // each part fixes its own x-positions of its row
             const bool wz = (g0 + t) == ar.n1[2];
-            if (xwrap | ywrap | wz) {
+            if (xwrap | ywrap | wz) {                                    // CTA-uniform
                 const bool wyy = ywrap && j == P;
-#pragma unroll 1
-                for (int a = 0; a < n; ++a) {
-                    const bool wx = xwrap && a == P;
-                    if (wx | wyy | wz) {
+#pragma unroll
+                for (int ii = 0; ii < NAH; ++ii) {
+                    const bool wx = xwrap && (A0 + ii == P);
+                    const double val = IN[Cfg::ofs(j, A0 + ii) + col];
+                    const double other = __shfl_xor_sync(0xffffffffu, val, 1);
+                    if ((wx | wyy | wz) && valid) {
                         double pr, pi; phase_of(ar, wx, wyy, wz, pr, pi);
-                        const double val = IN[(j * n + a) * C + col];
-                        const double other = __shfl_xor_sync(0xffffffffu, val, 1);
-                        IN[(j * n + a) * C + col] = ri == 0 ? val * pr - other * pi : other * pi + val * pr;
+                        IN[Cfg::ofs(j, A0 + ii) + col] = ri == 0 ? val * pr - other * pi : other * pi + val * pr;
                     }
                 }
-                asm volatile("bar.sync 1, %0;" ::"r"(n * 32) : "memory");   // consumer warps only
+                asm volatile("bar.sync 1, %0;" ::"r"(Cfg::CWARPS * 32) : "memory");   // consumer warps only
             }
         }
         const double* INc = IN + col;
         double row[n];
 #pragma unroll
-        for (int a = 0; a < n; ++a) row[a] = INc[(j * n + a) * C];
-        double ip[n];
-        // y-contraction: column a of the plane against row j of KY
+        for (int a = 0; a < n; ++a) row[a] = INc[Cfg::ofs(j, a)];
+        double ip[NAH];
+        // y-contraction: column A0 + ii of the plane against row j of KY
 #pragma unroll
-        for (int a = 0; a < n; ++a) {
+        for (int ii = 0; ii < NAH; ++ii) {
             double sy = 0.0;
 #pragma unroll
-            for (int b = 0; b < n; ++b) sy = fma(kyrow[b], INc[(b * n + a) * C], sy);
-            ip[a] = sc.WX[a] * sy;
+            for (int b = 0; b < n; ++b) sy = fma(kyrow[b], INc[Cfg::ofs(b, A0 + ii)], sy);
+            ip[ii] = sc.WX[A0 + ii] * sy;
         }
-        // x-contraction on the own row
+        // x-contraction on the own row, own outputs
 #pragma unroll
-        for (int i = 0; i < n; ++i) {
+        for (int ii = 0; ii < NAH; ++ii) {
             double sx = 0.0;
 #pragma unroll
-            for (int a = 0; a < n; ++a) sx = fma(sc.KX[i][a], row[a], sx);
-            ip[i] = fma(wyj, sx, ip[i]);
+            for (int a = 0; a < n; ++a) sx = fma(sc.KX[A0 + ii][a], row[a], sx);
+            ip[ii] = fma(wyj, sx, ip[ii]);
         }
-        double zr[n];
+        double zr[NAH];
 #pragma unroll
-        for (int a = 0; a < n; ++a) zr[a] = wxy[a] * row[a];
+        for (int ii = 0; ii < NAH; ++ii) zr[ii] = wxy[ii] * row[A0 + ii];
         if (lower) {
 #pragma unroll
             for (int k = 0; k < n; ++k)
 #pragma unroll
-                for (int a = 0; a < n; ++a) acc[k][a] = fma(sc.KZ[k][P], zr[a], acc[k][a]);
+                for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = fma(sc.KZ[k][P], zr[ii], acc[k][ii]);
 #pragma unroll
-            for (int a = 0; a < n; ++a) acc[P][a] = fma(sc.WZ[P], ip[a], acc[P][a]);
+            for (int ii = 0; ii < NAH; ++ii) acc[P][ii] = fma(sc.WZ[P], ip[ii], acc[P][ii]);
             // the previous cell is complete: emit its planes 0..P-1, carry its top plane over
             emit(ar, g0 + t - P, P);
 #pragma unroll
-            for (int a = 0; a < n; ++a) acc[0][a] = acc[P][a];
+            for (int ii = 0; ii < NAH; ++ii) acc[0][ii] = acc[P][ii];
 #pragma unroll
             for (int k = 1; k < n; ++k)
 #pragma unroll
-                for (int a = 0; a < n; ++a) acc[k][a] = 0.0;
+                for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = 0.0;
         }
         if (upper) {
             // z-push with the runtime cell-local index c: column c of KZ fetched from the constant bank
@@ -232,29 +266,32 @@ struct MarchConsumer {
             for (int k = 0; k < n; ++k) {
                 const double kz = sc.KZ[k][c];
 #pragma unroll
-                for (int a = 0; a < n; ++a) acc[k][a] = fma(kz, zr[a], acc[k][a]);
+                for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = fma(kz, zr[ii], acc[k][ii]);
             }
             const double wzc = sc.WZ[c];
 #pragma unroll
-            for (int a = 0; a < n; ++a) ip[a] *= wzc;
+            for (int ii = 0; ii < NAH; ++ii) ip[ii] *= wzc;
             if (jown) {
                 // S5 on the owned nodes of this plane (a < P): eq. 12 spin blocks, in-term, R-term
                 const double pz = sc.PZ[c] * pyj, fz = sc.FZ[c] * fyj * cin;
 #pragma unroll
-                for (int a = 0; a < P; ++a) {
-                    const double in_own = row[a];
-                    const double o_same = INc[(j * n + a) * C + ((col ^ 16) - col)];
-                    const double o_flip = INc[(j * n + a) * C + ((col ^ 17) - col)];
-                    const double u_re = ri == 0 ? o_same : o_flip;       // other spin, same vector
-                    const double u_im = ri == 0 ? o_flip : o_same;
-                    const double4 f = *reinterpret_cast<const double4*>(Fs + (j * P + a) * 4);
-                    const double diag = s_spin == 0 ? f.x : f.y;
-                    const double sy = s_spin == 0 ? -f.w : f.w;
-                    const double offd = ri == 0 ? f.z * u_re - sy * u_im : f.z * u_im + sy * u_re;
-                    double val = fma(pz * sc.PX[a], fma(diag, in_own, offd), ip[a]);
-                    val = fma(fz * sc.FX[a], in_own, val);
-                    if (ar.useR) val = fma(cR, Rs[(j * P + a) * C + col], val);
-                    ip[a] = val;
+                for (int ii = 0; ii < NAH; ++ii) {
+                    const int a = A0 + ii;
+                    if (a < P) {
+                        const double in_own = row[a];
+                        const double o_same = INc[Cfg::ofs(j, a) + ((col ^ (C / 2)) - col)];
+                        const double o_flip = INc[Cfg::ofs(j, a) + ((col ^ (C / 2 + 1)) - col)];
+                        const double u_re = ri == 0 ? o_same : o_flip;       // other spin, same vector
+                        const double u_im = ri == 0 ? o_flip : o_same;
+                        const double4 f = *reinterpret_cast<const double4*>(Fs + (j * P + a) * 4);
+                        const double diag = s_spin == 0 ? f.x : f.y;
+                        const double sy = s_spin == 0 ? -f.w : f.w;
+                        const double offd = ri == 0 ? f.z * u_re - sy * u_im : f.z * u_im + sy * u_re;
+                        double val = fma(pz * sc.PX[a], fma(diag, in_own, offd), ip[ii]);
+                        val = fma(fz * sc.FX[a], in_own, val);
+                        if (ar.useR) val = fma(cR, Rs[(j * P + a) * C + col], val);
+                        ip[ii] = val;
+                    }
                 }
             }
             // add the in-plane + pointwise part to the accumulator of the plane's own index
@@ -262,21 +299,40 @@ struct MarchConsumer {
             for (int k = 0; k < P; ++k) {
                 if (c == k) {
 #pragma unroll
-                    for (int a = 0; a < n; ++a) acc[k][a] += ip[a];
+                    for (int ii = 0; ii < NAH; ++ii) acc[k][ii] += ip[ii];
                 }
             }
         }
         __syncwarp();
-        if (col == 0) mbar_arrive(&empty_bar[s]);
+        if ((threadIdx.x & 31) == 0) mbar_arrive(&empty_bar[s]);
+    }
+
+    __device__ __forceinline__ void run(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, uint64_t* full_bar,
+                                        uint64_t* empty_bar, int T) {
+        int c = 0;
+#pragma unroll 1
+        for (int t = 0; t < T; ++t) {
+            plane(sc, ar, smem, full_bar, empty_bar, t, c, c == 0 && t > 0, t < T - 1);
+            c = (c + 1 == P) ? 0 : c + 1;
+        }
+        emit(ar, g0 + T - 1, 1);                                   // partial of the segment's top face
     }
 };
 
-template <int P, bool HASPH>
-__global__ void __launch_bounds__(MarchCfg<P>::THREADS, 1)
+template <int P, int CC, int XSPLIT, bool HASPH, int H>
+__device__ __forceinline__ void march_consume(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, uint64_t* full_bar,
+                                           uint64_t* empty_bar, int row, int col, int ex, int ey, int chunk, int g0, int T,
+                                           bool xwrap, bool ywrap) {
+    MarchConsumer<P, CC, XSPLIT, HASPH, H> cs;
+    cs.init(sc, ar, row, col, ex, ey, chunk, g0, xwrap, ywrap);
+    cs.run(sc, ar, smem, full_bar, empty_bar, T);
+}
+
+template <int P, int CC, int XSPLIT, bool HASPH>
+__global__ void __launch_bounds__(MarchCfg<P, CC, XSPLIT>::THREADS, 1)
 cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ MarchArgs ar,
-                  const __grid_constant__ CUtensorMap map_in_full, const __grid_constant__ CUtensorMap map_in_p,
-                  const __grid_constant__ CUtensorMap map_in_1, const __grid_constant__ CUtensorMap map_R) {
-    using Cfg = MarchCfg<P>;
+                  const __grid_constant__ MarchMaps mp) {
+    using Cfg = MarchCfg<P, CC, XSPLIT>;
     constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES;
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t full_bar[STAGES], empty_bar[STAGES];
@@ -293,15 +349,15 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
     const bool xwrap = ex == ar.nc[0] - 1, ywrap = ey == ar.nc[1] - 1;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], n); }
+        for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], Cfg::CWARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (warp == n) {
+    if (warp == Cfg::CWARPS) {
         // ================================ producer ================================
         if (lane == 0) {
-            const int col0 = chunk * 16;                          // doubles
+            const int col0 = chunk * (C / 2);                     // doubles
             for (int t = 0; t < T; ++t) {
                 const int s = t % STAGES;
                 const uint32_t par = (t / STAGES) & 1;
@@ -312,21 +368,22 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
                 mbar_expect_tx(&full_bar[s], bytes);
                 unsigned char* st = smem + (size_t)s * Cfg::STAGE_BYTES;
                 int gz = g0 + t; if (gz == ar.n1[2]) gz = 0;
-                for (int jj = 0; jj < n; ++jj) {
-                    int gy = ey * P + jj; if (gy == ar.n1[1]) gy = 0;
-                    const long long line0 = ((long long)gz * ar.n1[1] + gy) * ar.n1[0];   // node index of x = 0
-                    const long long node0 = line0 + (long long)ex * P;
-                    unsigned char* dst = st + jj * n * C * 8;
-                    if (!xwrap) {
-                        tma_load_2d(dst, &map_in_full, col0, (int)(2 * node0), &full_bar[s]);
-                    } else {
-                        tma_load_2d(dst, &map_in_p, col0, (int)(2 * node0), &full_bar[s]);
-                        tma_load_2d(dst + P * C * 8, &map_in_1, col0, (int)(2 * line0), &full_bar[s]);
-                    }
-                    if (owned && jj < P) {
-                        if (ar.useR) tma_load_2d(st + Cfg::R_OFF + jj * P * C * 8, &map_R, col0, (int)(2 * node0), &full_bar[s]);
-                        bulk_load(st + Cfg::F_OFF + jj * P * 32, ar.fields + node0 * 4, P * 32, &full_bar[s]);
-                    }
+                // lines ey*P .. ey*P+P of plane gz; the last one wraps to y = 0 in the last cell row
+                const int line = gz * ar.n1[1] + ey * P;
+                const int xr = 2 * ex * P;                                  // first (node, spin) row of the cell in its x-line
+                const int xf = xwrap ? 0 : xr + 2 * P;                       // rows of the x = P face column
+                if (!ywrap) {
+                    tma_load_3d(st, &mp.main[0], col0, xr, line, &full_bar[s]);
+                    tma_load_3d(st + Cfg::FACE_OFF, &mp.face[0], col0, xf, line, &full_bar[s]);
+                } else {
+                    tma_load_3d(st, &mp.main[1], col0, xr, line, &full_bar[s]);
+                    tma_load_3d(st + P * P * C * 8, &mp.main[2], col0, xr, gz * ar.n1[1], &full_bar[s]);
+                    tma_load_3d(st + Cfg::FACE_OFF, &mp.face[1], col0, xf, line, &full_bar[s]);
+                    tma_load_3d(st + Cfg::FACE_OFF + P * C * 8, &mp.face[2], col0, xf, gz * ar.n1[1], &full_bar[s]);
+                }
+                if (owned) {
+                    if (ar.useR) tma_load_3d(st + Cfg::R_OFF, &mp.R, col0, xr, line, &full_bar[s]);
+                    tma_load_2d(st + Cfg::F_OFF, &mp.F, 4 * ex * P, line, &full_bar[s]);
                 }
             }
         }
@@ -334,15 +391,15 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
     }
 
     // ================================ consumers ================================
-    MarchConsumer<P, HASPH> cs;
-    cs.init(sc, ar, warp, lane, ex, ey, chunk, g0, xwrap, ywrap);
-    int c = 0;
-#pragma unroll 1
-    for (int t = 0; t < T; ++t) {
-        cs.plane(sc, ar, smem, full_bar, empty_bar, t, c, c == 0 && t > 0, t < T - 1);
-        c = (c + 1 == P) ? 0 : c + 1;
-    }
-    cs.emit(ar, g0 + T - 1, 1);                                   // partial of the segment's top face
+    const int h = warp / Cfg::WPH;
+    const int row = (warp % Cfg::WPH) * Cfg::RPW + lane / C;
+    const int col = lane % C;
+#define MARCH_PART(HH)                                                                                              \
+    if (HH < XSPLIT && h == HH)                                                                                     \
+        march_consume<P, CC, XSPLIT, HASPH, (HH < XSPLIT ? HH : 0)>(sc, ar, smem, full_bar, empty_bar, row, col, ex, ey, \
+                                                                    chunk, g0, T, xwrap, ywrap);
+    MARCH_PART(0) MARCH_PART(1) MARCH_PART(2)
+#undef MARCH_PART
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -362,25 +419,43 @@ static EncodeFn get_encode() {
     return fn;
 }
 
-// 2-D view of a multivector: dim0 = 2*ld doubles of one (node, spin) row, dim1 = 2*M rows; box = 16 doubles x rows
-static bool make_map(CUtensorMap* map, const double* base, long long ld, long long nrows, int box_rows) {
+// 3-D view of a multivector: dim0 = 2*ld doubles of one (node, spin) row, dim1 = the 2*N1x rows of one x-line,
+// dim2 = the N1y*N1z x-lines; box = box_cols doubles x box_rows rows x box_lines lines
+static bool make_map3(CUtensorMap* map, const chfsi_mesh* m, const double* base, long long ld, int box_cols, int box_rows,
+                      int box_lines) {
     EncodeFn enc = get_encode();
     if (!enc) return false;
-    cuuint64_t gdim[2] = {(cuuint64_t)(2 * ld), (cuuint64_t)nrows};
-    cuuint64_t gstr[1] = {(cuuint64_t)(ld * 16)};
-    cuuint32_t box[2] = {16u, (cuuint32_t)box_rows};
-    cuuint32_t estr[2] = {1u, 1u};
-    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), gdim, gstr, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+    const cuuint64_t n1x = (cuuint64_t)m->mc.n1[0];
+    cuuint64_t gdim[3] = {(cuuint64_t)(2 * ld), 2 * n1x, (cuuint64_t)m->mc.n1[1] * (cuuint64_t)m->mc.n1[2]};
+    cuuint64_t gstr[2] = {(cuuint64_t)(ld * 16), 2 * n1x * (cuuint64_t)(ld * 16)};
+    cuuint32_t box[3] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows, (cuuint32_t)box_lines};
+    cuuint32_t estr[3] = {1u, 1u, 1u};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), gdim, gstr, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+               box_cols * 8 >= 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// 2-D view of the packed fields [M][4]: dim0 = the 4*N1x doubles of one x-line, dim1 = lines; box = 4P doubles x P lines
+static bool make_mapF(CUtensorMap* map, const chfsi_mesh* m, int P) {
+    EncodeFn enc = get_encode();
+    if (!enc) return false;
+    const cuuint64_t n1x = (cuuint64_t)m->mc.n1[0];
+    cuuint64_t gdim[2] = {4 * n1x, (cuuint64_t)m->mc.n1[1] * (cuuint64_t)m->mc.n1[2]};
+    cuuint64_t gstr[1] = {n1x * 32};
+    cuuint32_t box[2] = {(cuuint32_t)(4 * P), (cuuint32_t)P};
+    cuuint32_t estr[2] = {1u, 1u};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, m->dF, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 bool march_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a) {
     if (prec != CHFSI_FP64) return false;
-    if (m->p != 2 && m->p != 4 && m->p != 6) return false;
+    if (m->p != 2 && m->p != 4 && m->p != 6 && m->p != 8) return false;
     if (m->dF == nullptr) return false;
     // TMA needs 16-byte aligned bases/strides (always true for complex128 rows) and 32-bit row coordinates
     if (2 * m->nnodes >= (1ll << 31)) return false;
+    if (m->mc.n1[0] * 4ll * 8 % 16 != 0) return false;
     if (((uintptr_t)a.in & 15) || ((uintptr_t)a.out & 15) || (a.R && ((uintptr_t)a.R & 15))) return false;
     return get_encode() != nullptr;
 }
@@ -409,9 +484,9 @@ static void build_step_const(const chfsi_mesh* m, const CellArgs& a, StepConst& 
     }
 }
 
-template <int P>
+template <int P, int CC, int XSPLIT>
 static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaStream_t st) {
-    using Cfg = MarchCfg<P>;
+    using Cfg = MarchCfg<P, CC, XSPLIT>;
     StepConst sc;
     build_step_const(m, a, sc);
     MarchArgs ar;
@@ -421,7 +496,7 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
         ar.ph_re[d] = m->mc.ph_re[d]; ar.ph_im[d] = m->mc.ph_im[d];
     }
     ar.has_phase = m->mc.has_phase;
-    ar.nvec = a.nvec; ar.nchunks = (a.nvec + 7) / 8;
+    ar.nvec = a.nvec; ar.nchunks = (a.nvec + Cfg::NV - 1) / Cfg::NV;
     ar.useR = (a.R != nullptr && a.cR != nullptr) ? 1 : 0;
     ar.fields = m->dF; ar.cin = a.cin; ar.cR = a.cR; ar.out = a.out; ar.ld_out = a.ld_out;
     // z segmentation: enough CTAs for >= ~4 waves of one CTA per SM
@@ -430,15 +505,17 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
     for (int cand = 1; cand <= ar.nc[2]; ++cand)
         if (ar.nc[2] % cand == 0) { nseg = cand; if (base * cand >= 4 * 148) break; }
     ar.nseg = nseg; ar.cps = ar.nc[2] / nseg;
-    CUtensorMap mf, mp, m1, mr;
-    const long long rows = 2 * m->nnodes;
-    if (!make_map(&mf, a.in, a.ld_in, rows, 2 * (P + 1)) || !make_map(&mp, a.in, a.ld_in, rows, 2 * P) ||
-        !make_map(&m1, a.in, a.ld_in, rows, 2) ||
-        !make_map(&mr, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, rows, 2 * P))
+    MarchMaps mp;
+    constexpr int BC = CC / 2;
+    const int nl[3] = {P + 1, P, 1};
+    for (int i = 0; i < 3; ++i)
+        if (!make_map3(&mp.main[i], m, a.in, a.ld_in, BC, 2 * P, nl[i]) || !make_map3(&mp.face[i], m, a.in, a.ld_in, BC, 2, nl[i]))
+            return cudaErrorInvalidValue;
+    if (!make_map3(&mp.R, m, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, BC, 2 * P, P) || !make_mapF(&mp.F, m, P))
         return cudaErrorInvalidValue;
     const size_t smem = (size_t)Cfg::STAGES * Cfg::STAGE_BYTES;
-    static bool attr_done[128] = {false};
-    auto kern = m->mc.has_phase ? cell_march_kernel<P, true> : cell_march_kernel<P, false>;
+    static bool attr_done[128] = {false};   // per template instantiation
+    auto kern = m->mc.has_phase ? cell_march_kernel<P, CC, XSPLIT, true> : cell_march_kernel<P, CC, XSPLIT, false>;
     const int slot = (m->device & 63) * 2 + (m->mc.has_phase ? 1 : 0);
     if (!attr_done[slot]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -446,15 +523,16 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
         attr_done[slot] = true;
     }
     const long long grid = base * nseg;
-    kern<<<(unsigned)grid, Cfg::THREADS, smem, st>>>(sc, ar, mf, mp, m1, mr);
+    kern<<<(unsigned)grid, Cfg::THREADS, smem, st>>>(sc, ar, mp);
     return cudaGetLastError();
 }
 
 cudaError_t launch_cell_march(const chfsi_mesh* m, const CellArgs& a, cudaStream_t st) {
     switch (m->p) {
-        case 2: return launch_march_t<2>(m, a, st);
-        case 4: return launch_march_t<4>(m, a, st);
-        case 6: return launch_march_t<6>(m, a, st);
+        case 2: return launch_march_t<2, 32, 1>(m, a, st);
+        case 4: return launch_march_t<4, 32, 1>(m, a, st);
+        case 6: return launch_march_t<6, 32, 1>(m, a, st);
+        case 8: return launch_march_t<8, 16, 3>(m, a, st);
         default: return cudaErrorInvalidValue;
     }
 }
