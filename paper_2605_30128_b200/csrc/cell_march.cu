@@ -33,6 +33,11 @@ struct StepConst {
     double WX[kMaxN], WY[kMaxN], WZ[kMaxN];   // w * sout * sin per direction
     double PX[kMaxN], PY[kMaxN], PZ[kMaxN];   // product = cH * s_out * (u/in)   (potential coefficient)
     double FX[kMaxN], FY[kMaxN], FZ[kMaxN];   // product = in-term mass factor
+    // FP32 product (CHFSI_FP32): the same tables without cH, rounded once to FP32; cH is applied in FP64 when the
+    // FP32 Laplacian is widened
+    float KXf[kMaxN][kMaxN], KYf[kMaxN][kMaxN], KZf[kMaxN][kMaxN];
+    float WXf[kMaxN], WYf[kMaxN], WZf[kMaxN];
+    double cH;
 };
 
 struct MarchArgs {
@@ -114,6 +119,14 @@ struct MarchCfg {
     static constexpr int F_OFF = IN_BYTES + R_BYTES;
     static constexpr int STAGE_BYTES = ((F_OFF + F_BYTES + 127) / 128) * 128;
     static constexpr int STAGES = (200 * 1024 / STAGE_BYTES) < 8 ? (200 * 1024 / STAGE_BYTES) : 8;
+    // FP32 product: a ring of NFB FP32 copies of the gathered plane (written by the converter warp) and the
+    // per-thread FP64 pointwise store PW [P planes][P rows][P nodes][C] (recurrence terms stay FP64)
+    static constexpr int NFB = 3;
+    static constexpr int FB_BYTES = n * n * C * 4;
+    static constexpr int PW_BYTES = P * P * P * C * 8;
+    static constexpr int STAGES32_ = (200 * 1024 - PW_BYTES - NFB * FB_BYTES) / STAGE_BYTES;
+    static constexpr int STAGES32 = STAGES32_ < 8 ? STAGES32_ : 8;
+    static constexpr int THREADS32 = (CWARPS + 2) * 32;
 };
 
 // Per-thread state of a consumer (part H of row j, lane = batch column).
@@ -319,6 +332,230 @@ struct MarchConsumer {
     }
 };
 
+// ---------------------------------------------------------------------------------------------
+// FP32 product (CHFSI_FP32): the Laplacian of fl32(in) is computed and accumulated in FP32 from
+// the converter warp's FP32 copy of the plane; the pointwise potential, the in-term and the R-term of eq. 11 are
+// computed in FP64 from the FP64 stage and parked in the thread's own slots of PW until the cell is emitted, where
+// the FP32 Laplacian is widened exactly, scaled by cH in FP64 and both are sent out with one RED.ADD.F64.
+template <int P, int CC, int XSPLIT, bool HASPH, int H>
+struct MarchConsumerF32 {
+    using Cfg = MarchCfg<P, CC, XSPLIT>;
+    static constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES32, NFB = Cfg::NFB;
+    static constexpr int A0 = H * Cfg::NA;
+    static constexpr int NAH = (n - A0) < Cfg::NA ? (n - A0) : Cfg::NA;
+    float acc[n][NAH];
+    float kyrow[n], wxy[NAH];
+    float wyj;
+    double pyj, fyj, cin, cR;
+    double* outcol;
+    double* pw;                  // PW + (j * P) * C + col : this thread's pointwise slots, [c][.][a][.]
+    int j, col, s_spin, ri, ex, gy, g0;
+    bool vok, jown, wy, xwrap, ywrap, valid;
+
+    __device__ __forceinline__ void init(const StepConst& sc, const MarchArgs& ar, double* PW, int row, int col_, int ex_, int ey,
+                                         int chunk, int g0_, bool xw, bool yw) {
+        valid = row < n;
+        j = valid ? row : n - 1; col = col_; ex = ex_; g0 = g0_; xwrap = xw; ywrap = yw;
+        s_spin = col / (C / 2); ri = col & 1;
+        const int vl = (col % (C / 2)) >> 1;
+        const int v = chunk * Cfg::NV + vl;
+        vok = valid && v < ar.nvec;
+        jown = j < P;
+#pragma unroll
+        for (int b = 0; b < n; ++b) kyrow[b] = sc.KYf[j][b];
+#pragma unroll
+        for (int ii = 0; ii < NAH; ++ii) wxy[ii] = sc.WXf[A0 + ii] * sc.WYf[j];
+        wyj = sc.WYf[j]; pyj = sc.PY[j]; fyj = sc.FY[j];
+        cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
+        cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
+        gy = ey * P + j; wy = gy == ar.n1[1]; if (wy) gy = 0;
+        outcol = ar.out + ((long long)s_spin * ar.ld_out + (vok ? v : 0)) * 2 + ri;
+        pw = PW + (jown ? j : 0) * P * C + col;
+#pragma unroll
+        for (int k = 0; k < n; ++k)
+#pragma unroll
+            for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = 0.f;
+    }
+
+    __device__ __forceinline__ static void phase_of(const MarchArgs& ar, bool wx, bool wyy, bool wz, double& pr, double& pi) {
+        pr = 1.0; pi = 0.0;
+        if (wx) { pr = ar.ph_re[0]; pi = ar.ph_im[0]; }
+        if (wyy) { const double tt = pr * ar.ph_re[1] - pi * ar.ph_im[1]; pi = pr * ar.ph_im[1] + pi * ar.ph_re[1]; pr = tt; }
+        if (wz) { const double tt = pr * ar.ph_re[2] - pi * ar.ph_im[2]; pi = pr * ar.ph_im[2] + pi * ar.ph_re[2]; pr = tt; }
+    }
+
+    // emit planes [0, nk): out += cH * (double)acc + PW (owned nodes only; with_pw false for the segment's top face)
+    __device__ __forceinline__ void emit(const StepConst& sc, const MarchArgs& ar, int gzbase, int nk, bool with_pw) {
+        const long long xstride = 4 * ar.ld_out;
+        const long long x0 = (long long)ex * P + A0;
+#pragma unroll
+        for (int k = 0; k < n; ++k) {
+            if (k < nk) {
+                int gz = gzbase + k; const bool wz = gz == ar.n1[2]; if (wz) gz = 0;
+                double* line = outcol + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xstride;
+                double* pnode = line + x0 * xstride;
+#pragma unroll
+                for (int ii = 0; ii < NAH; ++ii) {
+                    const bool wx = (A0 + ii == P) && xwrap;
+                    double* dst = wx ? line : pnode + ii * xstride;
+                    double val = sc.cH * (double)acc[k][ii];
+                    if (A0 + ii < P && k < P) {
+                        if (with_pw && jown) val += pw[(k * P * P + A0 + ii) * C];
+                    }
+                    if (HASPH) {
+                        const double other = __shfl_xor_sync(0xffffffffu, val, 1);
+                        if (wx | wy | wz) {
+                            double pr, pi; phase_of(ar, wx, wy, wz, pr, pi);
+                            val = ri == 0 ? val * pr + other * pi : val * pr - other * pi;   // times conj(phase)
+                        }
+                    }
+                    if (vok) atomicAdd(dst, val);
+                }
+            }
+        }
+    }
+
+    __device__ __forceinline__ void plane(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, const float* FBbase,
+                                          uint64_t* full_bar, uint64_t* empty_bar, uint64_t* cfull_bar, uint64_t* cempty_bar,
+                                          int t, int c, bool lower, bool upper) {
+        const int s = t % STAGES, f = t % NFB;
+        mbar_wait(&cfull_bar[f], (t / NFB) & 1);
+        mbar_wait(&full_bar[s], (t / STAGES) & 1);           // already complete; orders this thread after the TMA writes
+        const double* INc = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES) + col;
+        const double* Rs = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES + Cfg::R_OFF);
+        const double* Fs = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES + Cfg::F_OFF);
+        const float* FBc = FBbase + (size_t)f * (Cfg::FB_BYTES / 4) + col;
+        float row[n];
+#pragma unroll
+        for (int a = 0; a < n; ++a) row[a] = FBc[Cfg::ofs(j, a)];
+        float ip[NAH];
+#pragma unroll
+        for (int ii = 0; ii < NAH; ++ii) {
+            float sy = 0.f;
+#pragma unroll
+            for (int b = 0; b < n; ++b) sy = fmaf(kyrow[b], FBc[Cfg::ofs(b, A0 + ii)], sy);
+            ip[ii] = sc.WXf[A0 + ii] * sy;
+        }
+#pragma unroll
+        for (int ii = 0; ii < NAH; ++ii) {
+            float sx = 0.f;
+#pragma unroll
+            for (int a = 0; a < n; ++a) sx = fmaf(sc.KXf[A0 + ii][a], row[a], sx);
+            ip[ii] = fmaf(wyj, sx, ip[ii]);
+        }
+        float zr[NAH];
+#pragma unroll
+        for (int ii = 0; ii < NAH; ++ii) zr[ii] = wxy[ii] * row[A0 + ii];
+        if (lower) {
+#pragma unroll
+            for (int k = 0; k < n; ++k)
+#pragma unroll
+                for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = fmaf(sc.KZf[k][P], zr[ii], acc[k][ii]);
+#pragma unroll
+            for (int ii = 0; ii < NAH; ++ii) acc[P][ii] = fmaf(sc.WZf[P], ip[ii], acc[P][ii]);
+            emit(sc, ar, g0 + t - P, P, true);
+#pragma unroll
+            for (int ii = 0; ii < NAH; ++ii) acc[0][ii] = acc[P][ii];
+#pragma unroll
+            for (int k = 1; k < n; ++k)
+#pragma unroll
+                for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = 0.f;
+        }
+        if (upper) {
+#pragma unroll
+            for (int k = 0; k < n; ++k) {
+                const float kz = sc.KZf[k][c];
+#pragma unroll
+                for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = fmaf(kz, zr[ii], acc[k][ii]);
+            }
+            const float wzc = sc.WZf[c];
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                if (c == k) {
+#pragma unroll
+                    for (int ii = 0; ii < NAH; ++ii) acc[k][ii] = fmaf(wzc, ip[ii], acc[k][ii]);
+                }
+            }
+            if (jown) {
+                // S5 in FP64 on the owned nodes of this plane: eq. 12 spin blocks, in-term, R-term -> PW[c][j][a]
+                const double pz = sc.PZ[c] * pyj, fz = sc.FZ[c] * fyj * cin;
+                double* pwc = pw + c * P * P * C;
+#pragma unroll
+                for (int ii = 0; ii < NAH; ++ii) {
+                    const int a = A0 + ii;
+                    if (a < P) {
+                        const double in_own = INc[Cfg::ofs(j, a)];
+                        const double o_same = INc[Cfg::ofs(j, a) + ((col ^ (C / 2)) - col)];
+                        const double o_flip = INc[Cfg::ofs(j, a) + ((col ^ (C / 2 + 1)) - col)];
+                        const double u_re = ri == 0 ? o_same : o_flip;
+                        const double u_im = ri == 0 ? o_flip : o_same;
+                        const double4 fl = *reinterpret_cast<const double4*>(Fs + (j * P + a) * 4);
+                        const double diag = s_spin == 0 ? fl.x : fl.y;
+                        const double sy = s_spin == 0 ? -fl.w : fl.w;
+                        const double offd = ri == 0 ? fl.z * u_re - sy * u_im : fl.z * u_im + sy * u_re;
+                        double val = (pz * sc.PX[a]) * fma(diag, in_own, offd);
+                        val = fma(fz * sc.FX[a], in_own, val);
+                        if (ar.useR) val = fma(cR, Rs[(j * P + a) * C + col], val);
+                        pwc[a * C] = val;
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) { mbar_arrive(&empty_bar[s]); mbar_arrive(&cempty_bar[f]); }
+    }
+
+    __device__ __forceinline__ void run(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, const float* FBbase,
+                                        uint64_t* full_bar, uint64_t* empty_bar, uint64_t* cfull_bar, uint64_t* cempty_bar, int T) {
+        int c = 0;
+#pragma unroll 1
+        for (int t = 0; t < T; ++t) {
+            plane(sc, ar, smem, FBbase, full_bar, empty_bar, cfull_bar, cempty_bar, t, c, c == 0 && t > 0, t < T - 1);
+            c = (c + 1 == P) ? 0 : c + 1;
+        }
+        emit(sc, ar, g0 + T - 1, 1, false);
+    }
+};
+
+// Converter warp of the FP32 product: fl32 of the gathered plane (one RN cast per value, north_star (5): conversion
+// fused into the load path), with the Bloch phase of wrapped entries applied in FP64 before the cast.
+template <int P, int CC, int XSPLIT, bool HASPH>
+__device__ __forceinline__ void march_convert(const MarchArgs& ar, unsigned char* smem, float* FBbase, uint64_t* full_bar,
+                                              uint64_t* cfull_bar, uint64_t* cempty_bar, int lane, int g0, int T, bool xwrap,
+                                              bool ywrap) {
+    using Cfg = MarchCfg<P, CC, XSPLIT>;
+    constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES32, NFB = Cfg::NFB, HC = C / 2;
+#pragma unroll 1
+    for (int t = 0; t < T; ++t) {
+        const int s = t % STAGES, f = t % NFB;
+        mbar_wait(&cempty_bar[f], ((t / NFB) & 1) ^ 1);
+        mbar_wait(&full_bar[s], (t / STAGES) & 1);
+        const double2* IN2 = reinterpret_cast<const double2*>(smem + (size_t)s * Cfg::STAGE_BYTES);
+        float2* FB2 = reinterpret_cast<float2*>(FBbase + (size_t)f * (Cfg::FB_BYTES / 4));
+        const bool wz = HASPH && (g0 + t) == ar.n1[2];
+#pragma unroll 4
+        for (int e = lane; e < n * n * HC; e += 32) {
+            double2 v = IN2[e];
+            if (HASPH) {
+                const int sl = e / HC;                               // slot: MAIN [b][a < P] then FACE [b]
+                const bool face = sl >= n * P;
+                const int b = face ? sl - n * P : sl / P;
+                const bool wx = xwrap && face, wyy = ywrap && b == P;
+                if (wx | wyy | wz) {
+                    double pr = 1.0, pi = 0.0;
+                    if (wx) { pr = ar.ph_re[0]; pi = ar.ph_im[0]; }
+                    if (wyy) { const double tt = pr * ar.ph_re[1] - pi * ar.ph_im[1]; pi = pr * ar.ph_im[1] + pi * ar.ph_re[1]; pr = tt; }
+                    if (wz) { const double tt = pr * ar.ph_re[2] - pi * ar.ph_im[2]; pi = pr * ar.ph_im[2] + pi * ar.ph_re[2]; pr = tt; }
+                    v = make_double2(v.x * pr - v.y * pi, v.x * pi + v.y * pr);
+                }
+            }
+            FB2[e] = make_float2((float)v.x, (float)v.y);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&cfull_bar[f]);
+    }
+}
+
 template <int P, int CC, int XSPLIT, bool HASPH, int H>
 __device__ __forceinline__ void march_consume(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, uint64_t* full_bar,
                                            uint64_t* empty_bar, int row, int col, int ex, int ey, int chunk, int g0, int T,
@@ -328,14 +565,26 @@ __device__ __forceinline__ void march_consume(const StepConst& sc, const MarchAr
     cs.run(sc, ar, smem, full_bar, empty_bar, T);
 }
 
-template <int P, int CC, int XSPLIT, bool HASPH>
-__global__ void __launch_bounds__(MarchCfg<P, CC, XSPLIT>::THREADS, 1)
+template <int P, int CC, int XSPLIT, bool HASPH, int H>
+__device__ __forceinline__ void march_consume32(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, float* FB, double* PW,
+                                                uint64_t* full_bar, uint64_t* empty_bar, uint64_t* cfull_bar, uint64_t* cempty_bar,
+                                                int row, int col, int ex, int ey, int chunk, int g0, int T, bool xwrap, bool ywrap) {
+    MarchConsumerF32<P, CC, XSPLIT, HASPH, H> cs;
+    cs.init(sc, ar, PW, row, col, ex, ey, chunk, g0, xwrap, ywrap);
+    cs.run(sc, ar, smem, FB, full_bar, empty_bar, cfull_bar, cempty_bar, T);
+}
+
+template <int P, int CC, int XSPLIT, bool HASPH, bool F32>
+__global__ void __launch_bounds__(F32 ? MarchCfg<P, CC, XSPLIT>::THREADS32 : MarchCfg<P, CC, XSPLIT>::THREADS, 1)
 cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ MarchArgs ar,
                   const __grid_constant__ MarchMaps mp) {
     using Cfg = MarchCfg<P, CC, XSPLIT>;
-    constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES;
+    constexpr int n = Cfg::n, C = Cfg::C, STAGES = F32 ? Cfg::STAGES32 : Cfg::STAGES, NFB = Cfg::NFB;
     extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ __align__(8) uint64_t full_bar[STAGES], empty_bar[STAGES];
+    __shared__ __align__(8) uint64_t full_bar[STAGES], empty_bar[STAGES], cfull_bar[NFB], cempty_bar[NFB];
+    float* FB = reinterpret_cast<float*>(smem + (size_t)STAGES * Cfg::STAGE_BYTES);
+    double* PW = reinterpret_cast<double*>(smem + (size_t)STAGES * Cfg::STAGE_BYTES + NFB * Cfg::FB_BYTES);
+    (void)n; (void)FB; (void)PW;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // blockIdx -> (ex fastest, ey, seg, chunk): neighbours in x/y run together, so shared faces hit in L2
@@ -350,6 +599,7 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], Cfg::CWARPS); }
+        for (int f = 0; f < NFB; ++f) { mbar_init(&cfull_bar[f], 1); mbar_init(&cempty_bar[f], Cfg::CWARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -390,14 +640,25 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
         return;
     }
 
+    if (F32 && warp == Cfg::CWARPS + 1) {
+        march_convert<P, CC, XSPLIT, HASPH>(ar, smem, FB, full_bar, cfull_bar, cempty_bar, lane, g0, T, xwrap, ywrap);
+        return;
+    }
+
     // ================================ consumers ================================
     const int h = warp / Cfg::WPH;
     const int row = (warp % Cfg::WPH) * Cfg::RPW + lane / C;
     const int col = lane % C;
 #define MARCH_PART(HH)                                                                                              \
-    if (HH < XSPLIT && h == HH)                                                                                     \
-        march_consume<P, CC, XSPLIT, HASPH, (HH < XSPLIT ? HH : 0)>(sc, ar, smem, full_bar, empty_bar, row, col, ex, ey, \
-                                                                    chunk, g0, T, xwrap, ywrap);
+    if (HH < XSPLIT && h == HH) {                                                                                   \
+        if (F32)                                                                                                    \
+            march_consume32<P, CC, XSPLIT, HASPH, (HH < XSPLIT ? HH : 0)>(sc, ar, smem, FB, PW, full_bar, empty_bar, \
+                                                                          cfull_bar, cempty_bar, row, col, ex, ey,  \
+                                                                          chunk, g0, T, xwrap, ywrap);              \
+        else                                                                                                        \
+            march_consume<P, CC, XSPLIT, HASPH, (HH < XSPLIT ? HH : 0)>(sc, ar, smem, full_bar, empty_bar, row, col, ex, ey, \
+                                                                        chunk, g0, T, xwrap, ywrap);               \
+    }
     MARCH_PART(0) MARCH_PART(1) MARCH_PART(2)
 #undef MARCH_PART
 }
@@ -450,7 +711,7 @@ static bool make_mapF(CUtensorMap* map, const chfsi_mesh* m, int P) {
 }
 
 bool march_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a) {
-    if (prec != CHFSI_FP64) return false;
+    if (prec != CHFSI_FP64 && prec != CHFSI_FP32) return false;
     if (m->p != 2 && m->p != 4 && m->p != 6 && m->p != 8) return false;
     if (m->dF == nullptr) return false;
     // TMA needs 16-byte aligned bases/strides (always true for complex128 rows) and 32-bit row coordinates
@@ -465,6 +726,7 @@ static void build_step_const(const chfsi_mesh* m, const CellArgs& a, StepConst& 
     const int n = mc.n;
     const bool sin_ = (a.flags & kScaleIn) != 0, sout_ = (a.flags & kSoutInvM) != 0, massin = (a.flags & kMassIn) != 0;
     std::memset(&sc, 0, sizeof(sc));
+    sc.cH = a.cH;
     for (int d = 0; d < 3; ++d) {
         double (*K)[kMaxN] = d == 0 ? sc.KX : d == 1 ? sc.KY : sc.KZ;
         double* W = d == 0 ? sc.WX : d == 1 ? sc.WY : sc.WZ;
@@ -475,8 +737,10 @@ static void build_step_const(const chfsi_mesh* m, const CellArgs& a, StepConst& 
             for (int b = 0; b < n; ++b) {
                 const double sb = sin_ ? mc.im1[d][b] : 1.0;
                 K[i][b] = a.cH * so * mc.Kd[d][i][b] * sb;
+                (d == 0 ? sc.KXf : d == 1 ? sc.KYf : sc.KZf)[i][b] = (float)(so * mc.Kd[d][i][b] * sb);
             }
             W[i] = mc.w[i] * so * si;
+            (d == 0 ? sc.WXf : d == 1 ? sc.WYf : sc.WZf)[i] = (float)W[i];
             const double fu = sin_ ? 1.0 : mc.m1[d][i];                // u = m w: Z-form u = in, else m * in
             Pp[i] = so * fu * (d == 0 ? a.cH : 1.0);
             Fp[i] = massin ? mc.m1[d][i] : 1.0;
@@ -484,7 +748,7 @@ static void build_step_const(const chfsi_mesh* m, const CellArgs& a, StepConst& 
     }
 }
 
-template <int P, int CC, int XSPLIT>
+template <int P, int CC, int XSPLIT, bool F32>
 static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaStream_t st) {
     using Cfg = MarchCfg<P, CC, XSPLIT>;
     StepConst sc;
@@ -513,9 +777,10 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
             return cudaErrorInvalidValue;
     if (!make_map3(&mp.R, m, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, BC, 2 * P, P) || !make_mapF(&mp.F, m, P))
         return cudaErrorInvalidValue;
-    const size_t smem = (size_t)Cfg::STAGES * Cfg::STAGE_BYTES;
+    const size_t smem = F32 ? (size_t)Cfg::STAGES32 * Cfg::STAGE_BYTES + Cfg::NFB * Cfg::FB_BYTES + Cfg::PW_BYTES
+                            : (size_t)Cfg::STAGES * Cfg::STAGE_BYTES;
     static bool attr_done[128] = {false};   // per template instantiation
-    auto kern = m->mc.has_phase ? cell_march_kernel<P, CC, XSPLIT, true> : cell_march_kernel<P, CC, XSPLIT, false>;
+    auto kern = m->mc.has_phase ? cell_march_kernel<P, CC, XSPLIT, true, F32> : cell_march_kernel<P, CC, XSPLIT, false, F32>;
     const int slot = (m->device & 63) * 2 + (m->mc.has_phase ? 1 : 0);
     if (!attr_done[slot]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -523,16 +788,17 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
         attr_done[slot] = true;
     }
     const long long grid = base * nseg;
-    kern<<<(unsigned)grid, Cfg::THREADS, smem, st>>>(sc, ar, mp);
+    kern<<<(unsigned)grid, F32 ? Cfg::THREADS32 : Cfg::THREADS, smem, st>>>(sc, ar, mp);
     return cudaGetLastError();
 }
 
-cudaError_t launch_cell_march(const chfsi_mesh* m, const CellArgs& a, cudaStream_t st) {
+cudaError_t launch_cell_march(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t st) {
+    const bool f32 = prec == CHFSI_FP32;
     switch (m->p) {
-        case 2: return launch_march_t<2, 32, 1>(m, a, st);
-        case 4: return launch_march_t<4, 32, 1>(m, a, st);
-        case 6: return launch_march_t<6, 32, 1>(m, a, st);
-        case 8: return launch_march_t<8, 16, 3>(m, a, st);
+        case 2: return f32 ? launch_march_t<2, 32, 1, true>(m, a, st) : launch_march_t<2, 32, 1, false>(m, a, st);
+        case 4: return f32 ? launch_march_t<4, 32, 1, true>(m, a, st) : launch_march_t<4, 32, 1, false>(m, a, st);
+        case 6: return f32 ? launch_march_t<6, 32, 1, true>(m, a, st) : launch_march_t<6, 32, 1, false>(m, a, st);
+        case 8: return f32 ? launch_march_t<8, 16, 3, true>(m, a, st) : launch_march_t<8, 16, 3, false>(m, a, st);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -134,7 +134,7 @@ cudaError_t launch_coef(const double* hdr, double* table, int nrows, int nvec, c
 bool cell_supported(int p, chfsi_prec prec);
 // z-marching TMA kernel (cell_march.cu)
 bool march_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
-cudaError_t launch_cell_march(const chfsi_mesh* m, const CellArgs& a, cudaStream_t s);
+cudaError_t launch_cell_march(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
 void set_error(const std::string& s);
 void count_launch(int n = 1);
 }  // namespace chfsi

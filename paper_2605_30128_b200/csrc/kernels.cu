@@ -403,7 +403,7 @@ cudaError_t launch_cell(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a,
         cudaEventRecord(e0, st);
     }
     cudaError_t err;
-    if (!use_legacy() && march_supported(m, prec, a)) err = launch_cell_march(m, a, st);
+    if (!use_legacy() && march_supported(m, prec, a)) err = launch_cell_march(m, prec, a, st);
     else err = launch_cell_legacy(m, prec, a, st);
     count_launch();
     if (m->prof_on) {
