@@ -126,7 +126,8 @@ struct MarchCfg {
     static constexpr int PW_BYTES = P * P * P * C * 8;
     static constexpr int STAGES32_ = (200 * 1024 - PW_BYTES - NFB * FB_BYTES) / STAGE_BYTES;
     static constexpr int STAGES32 = STAGES32_ < 8 ? STAGES32_ : 8;
-    static constexpr int THREADS32 = (CWARPS + 2) * 32;
+    static constexpr int NCW = 4;                         // converter warps
+    static constexpr int THREADS32 = (CWARPS + 1 + NCW) * 32;
 };
 
 // Per-thread state of a consumer (part H of row j, lane = batch column).
@@ -521,8 +522,8 @@ struct MarchConsumerF32 {
 // fused into the load path), with the Bloch phase of wrapped entries applied in FP64 before the cast.
 template <int P, int CC, int XSPLIT, bool HASPH>
 __device__ __forceinline__ void march_convert(const MarchArgs& ar, unsigned char* smem, float* FBbase, uint64_t* full_bar,
-                                              uint64_t* cfull_bar, uint64_t* cempty_bar, int lane, int g0, int T, bool xwrap,
-                                              bool ywrap) {
+                                              uint64_t* cfull_bar, uint64_t* cempty_bar, int cw, int lane, int g0, int T,
+                                              bool xwrap, bool ywrap) {
     using Cfg = MarchCfg<P, CC, XSPLIT>;
     constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES32, NFB = Cfg::NFB, HC = C / 2;
 #pragma unroll 1
@@ -534,7 +535,7 @@ __device__ __forceinline__ void march_convert(const MarchArgs& ar, unsigned char
         float2* FB2 = reinterpret_cast<float2*>(FBbase + (size_t)f * (Cfg::FB_BYTES / 4));
         const bool wz = HASPH && (g0 + t) == ar.n1[2];
 #pragma unroll 4
-        for (int e = lane; e < n * n * HC; e += 32) {
+        for (int e = cw * 32 + lane; e < n * n * HC; e += 32 * Cfg::NCW) {
             double2 v = IN2[e];
             if (HASPH) {
                 const int sl = e / HC;                               // slot: MAIN [b][a < P] then FACE [b]
@@ -599,7 +600,7 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], Cfg::CWARPS); }
-        for (int f = 0; f < NFB; ++f) { mbar_init(&cfull_bar[f], 1); mbar_init(&cempty_bar[f], Cfg::CWARPS); }
+        for (int f = 0; f < NFB; ++f) { mbar_init(&cfull_bar[f], Cfg::NCW); mbar_init(&cempty_bar[f], Cfg::CWARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -640,8 +641,9 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
         return;
     }
 
-    if (F32 && warp == Cfg::CWARPS + 1) {
-        march_convert<P, CC, XSPLIT, HASPH>(ar, smem, FB, full_bar, cfull_bar, cempty_bar, lane, g0, T, xwrap, ywrap);
+    if (F32 && warp > Cfg::CWARPS) {
+        march_convert<P, CC, XSPLIT, HASPH>(ar, smem, FB, full_bar, cfull_bar, cempty_bar, warp - Cfg::CWARPS - 1, lane, g0, T,
+                                            xwrap, ywrap);
         return;
     }
 
