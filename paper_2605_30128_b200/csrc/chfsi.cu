@@ -93,7 +93,7 @@ static cudaError_t upload(T** dst, const std::vector<T>& src) {
 }
 
 static void free_nonlocal(NonlocalDev& nl) {
-    cudaFree(nl.items); cudaFree(nl.supp_node); cudaFree(nl.supp_mass); cudaFree(nl.p_off); cudaFree(nl.s_off);
+    cudaFree(nl.items); cudaFree(nl.items_big); cudaFree(nl.supp_node); cudaFree(nl.supp_mass); cudaFree(nl.p_off); cudaFree(nl.s_off);
     cudaFree(nl.nproj); cudaFree(nl.c_off); cudaFree(nl.d_off); cudaFree(nl.P64); cudaFree(nl.P32); cudaFree(nl.D64);
     nl = NonlocalDev();
 }
@@ -321,6 +321,16 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
                 items.push_back(ProjItem{a, (int)st, (int)((ns - st) < kSlice ? (ns - st) : kSlice)});
         }
         nl.nitems = (int)items.size();
+        std::vector<ProjItem> big;
+        constexpr int kBig = 32;     // must match kernels.cu
+        for (int a = 0; a < natoms; ++a) {
+            const long long ns = supp_off[a + 1] - supp_off[a];
+            for (long long st = 0; st < ns; st += kBig)
+                big.push_back(ProjItem{a, (int)st, (int)((ns - st) < kBig ? (ns - st) : kBig)});
+        }
+        nl.nitems_big = (int)big.size();
+        nl.uniform_np = nproj[0];
+        for (int a = 1; a < natoms; ++a) if (nproj[a] != nproj[0]) nl.uniform_np = 0;
         std::vector<long long> nodes(supp_node, supp_node + nnz);
         std::vector<double> smass(nnz);
         for (long long j = 0; j < nnz; ++j) smass[j] = node_mass(m, nodes[j]);
@@ -334,6 +344,7 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
         for (long long j = 0; j < dcount; ++j) D64[j] = make_double2(D[2 * j], D[2 * j + 1]);
         std::vector<int> np(nproj, nproj + natoms);
         CU(upload(&nl.items, items));
+        CU(upload(&nl.items_big, big));
         CU(upload(&nl.supp_node, nodes));
         CU(upload(&nl.supp_mass, smass));
         CU(upload(&nl.p_off, p_off));

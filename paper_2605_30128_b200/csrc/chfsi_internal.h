@@ -60,7 +60,10 @@ struct NonlocalDev {
     int nitems = 0;
     int max_nproj = 0;
     long long nnz = 0;                  // total support entries
-    ProjItem* items = nullptr;          // [nitems]
+    ProjItem* items = nullptr;          // [nitems]   slices of 8 support nodes
+    int nitems_big = 0;
+    int uniform_np = 0;                 // nproj if every atom has the same number of projectors, else 0
+    ProjItem* items_big = nullptr;      // [nitems_big] slices of 32 support nodes (fast kernels)
     long long* supp_node = nullptr;     // [nnz]
     double* supp_mass = nullptr;        // [nnz] m_I of each support entry
     long long* p_off = nullptr;         // [natoms] offset (in complex elements) of atom's P block

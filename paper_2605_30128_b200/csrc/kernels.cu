@@ -307,6 +307,129 @@ back_kernel(const NonlocalDev nl, const BackArgs ar) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Fast S4 path when every atom has the same NP projectors (NP = 4 or 8; the BASELINE configs): items of up to
+// kBig = 32 support nodes, the item's projector block, node list and masses staged in shared memory once, the
+// coefficients of one (spin, vector) column kept in registers across the item, so that C receives one RED per
+// coefficient and item (4x fewer than the 8-node slices above) and all loads of a batch are in flight together.
+// back_fast also forms its rows of G = D_a C_a itself (D_a in shared memory), which removes the gmat launch.
+constexpr int kBig = 32;
+
+template <typename TT> struct P2Sel;
+template <> struct P2Sel<double> { using type = double2; static __device__ __forceinline__ const double2* ptr(const NonlocalDev& nl) { return nl.P64; } };
+template <> struct P2Sel<float> { using type = float2; static __device__ __forceinline__ const float2* ptr(const NonlocalDev& nl) { return nl.P32; } };
+
+template <typename TT, int NP>
+__global__ void __launch_bounds__(128)
+proj_fast_kernel(const NonlocalDev nl, const ProjArgs ar) {
+    using P2 = typename P2Sel<TT>::type;
+    __shared__ P2 Ps[kBig * NP];
+    __shared__ long long nodes[kBig];
+    __shared__ double mass[kBig];
+    const ProjItem it = nl.items_big[blockIdx.x];
+    const long long soff = nl.s_off[it.atom] + it.start;
+    const long long poff = nl.p_off[it.atom] + (long long)it.start * NP;
+    for (int i = threadIdx.x; i < it.count * NP; i += 128) Ps[i] = P2Sel<TT>::ptr(nl)[poff + i];
+    if (threadIdx.x < kBig) {
+        const int jj = threadIdx.x < it.count ? threadIdx.x : 0;
+        nodes[threadIdx.x] = nl.supp_node[soff + jj];
+        mass[threadIdx.x] = ar.mass_u ? nl.supp_mass[soff + jj] : 1.0;
+    }
+    __syncthreads();
+    const int s = blockIdx.y & 1;
+    const int v = (blockIdx.y >> 1) * 128 + threadIdx.x;
+    if (v >= ar.nvec) return;
+    TT cr[NP], ci[NP];
+#pragma unroll
+    for (int b = 0; b < NP; ++b) { cr[b] = 0; ci[b] = 0; }
+    const double2* in2 = reinterpret_cast<const double2*>(ar.in) + (long long)s * ar.ld_in + v;
+#pragma unroll 1
+    for (int j0 = 0; j0 < it.count; j0 += kSlice) {
+        double2 x[kSlice];
+#pragma unroll
+        for (int jj = 0; jj < kSlice; ++jj) {
+            const bool ok = j0 + jj < it.count;
+            x[jj] = ok ? __ldg(in2 + 2 * nodes[j0 + jj] * ar.ld_in) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int jj = 0; jj < kSlice; ++jj) {
+            if (j0 + jj < it.count) {
+                const double m = mass[j0 + jj];
+                const TT xr = (TT)(x[jj].x * m), xi = (TT)(x[jj].y * m);
+#pragma unroll
+                for (int b = 0; b < NP; ++b) {
+                    const P2 pv = Ps[(j0 + jj) * NP + b];
+                    cr[b] = fma(pv.x, xr, fma(pv.y, xi, cr[b]));         // conj(p) x
+                    ci[b] = fma(pv.x, xi, fma(-pv.y, xr, ci[b]));
+                }
+            }
+        }
+    }
+    double* Crow = ar.C + (nl.c_off[it.atom] * (long long)ar.nvec + v) * 2;
+#pragma unroll
+    for (int b = 0; b < NP; ++b) {
+        double* dst = Crow + (long long)(2 * b + s) * ar.nvec * 2;
+        red_add(dst, (double)cr[b]);
+        red_add(dst + 1, (double)ci[b]);
+    }
+}
+
+template <typename TT, int NP>
+__global__ void __launch_bounds__(128)
+back_fast_kernel(const NonlocalDev nl, const BackArgs ar) {
+    using P2 = typename P2Sel<TT>::type;
+    __shared__ P2 Ps[kBig * NP];
+    __shared__ double2 Ds[2 * NP * 2 * NP];
+    __shared__ long long nodes[kBig];
+    __shared__ double fac[kBig];
+    const ProjItem it = nl.items_big[blockIdx.x];
+    const long long soff = nl.s_off[it.atom] + it.start;
+    const long long poff = nl.p_off[it.atom] + (long long)it.start * NP;
+    for (int i = threadIdx.x; i < it.count * NP; i += 128) Ps[i] = P2Sel<TT>::ptr(nl)[poff + i];
+    for (int i = threadIdx.x; i < 4 * NP * NP; i += 128) Ds[i] = nl.D64[nl.d_off[it.atom] + i];
+    if (threadIdx.x < kBig) {
+        const int jj = threadIdx.x < it.count ? threadIdx.x : 0;
+        nodes[threadIdx.x] = nl.supp_node[soff + jj];
+        fac[threadIdx.x] = ar.cH * (ar.sout_invm ? 1.0 : nl.supp_mass[soff + jj]);
+    }
+    __syncthreads();
+    const int s = blockIdx.y & 1;
+    const int v = (blockIdx.y >> 1) * 128 + threadIdx.x;
+    if (v >= ar.nvec) return;
+    // rows 2b + s of G = D C for this column (FP64: the coupling matrix is applied in double in every mode)
+    const double2* Cc = reinterpret_cast<const double2*>(ar.C) + nl.c_off[it.atom] * (long long)ar.nvec + v;
+    double gr[NP], gi[NP];
+#pragma unroll
+    for (int b = 0; b < NP; ++b) { gr[b] = 0.0; gi[b] = 0.0; }
+#pragma unroll 4
+    for (int r = 0; r < 2 * NP; ++r) {
+        const double2 cv = Cc[(long long)r * ar.nvec];
+#pragma unroll
+        for (int b = 0; b < NP; ++b) {
+            const double2 d = Ds[(2 * b + s) * 2 * NP + r];
+            gr[b] = fma(d.x, cv.x, fma(-d.y, cv.y, gr[b]));
+            gi[b] = fma(d.x, cv.y, fma(d.y, cv.x, gi[b]));
+        }
+    }
+    TT g_r[NP], g_i[NP];
+#pragma unroll
+    for (int b = 0; b < NP; ++b) { g_r[b] = (TT)gr[b]; g_i[b] = (TT)gi[b]; }
+    double* out = ar.out + ((long long)s * ar.ld_out + v) * 2;
+#pragma unroll 4
+    for (int jj = 0; jj < it.count; ++jj) {
+        TT yr = 0, yi = 0;
+#pragma unroll
+        for (int b = 0; b < NP; ++b) {
+            const P2 pv = Ps[jj * NP + b];
+            yr = fma(pv.x, g_r[b], fma(-pv.y, g_i[b], yr));
+            yi = fma(pv.x, g_i[b], fma(pv.y, g_r[b], yi));
+        }
+        double* dst = out + 4 * nodes[jj] * ar.ld_out;
+        red_add(dst, fac[jj] * (double)yr);
+        red_add(dst + 1, fac[jj] * (double)yi);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // S7 / scaled copies: out[row][v] = ca[v] * (a_inv_mass ? A/m : A) + cb[v] * B
 __global__ void __launch_bounds__(256)
 axpby_kernel(const __grid_constant__ MeshConst mc, double2* __restrict__ out, long long ldo,
@@ -435,6 +558,19 @@ static cudaError_t launch_cell_legacy(const chfsi_mesh* m, chfsi_prec prec, cons
 
 cudaError_t launch_proj(const chfsi_mesh* m, chfsi_prec prec, const ProjArgs& a, cudaStream_t st) {
     if (m->nl.nitems == 0) return cudaSuccess;
+    if (m->nl.uniform_np == 4 || m->nl.uniform_np == 8) {
+        dim3 grid(m->nl.nitems_big, 2 * ((a.nvec + 127) / 128));
+        const bool f32 = prec == CHFSI_FP32;
+        if (m->nl.uniform_np == 8) {
+            if (f32) proj_fast_kernel<float, 8><<<grid, 128, 0, st>>>(m->nl, a);
+            else proj_fast_kernel<double, 8><<<grid, 128, 0, st>>>(m->nl, a);
+        } else {
+            if (f32) proj_fast_kernel<float, 4><<<grid, 128, 0, st>>>(m->nl, a);
+            else proj_fast_kernel<double, 4><<<grid, 128, 0, st>>>(m->nl, a);
+        }
+        count_launch();
+        return cudaGetLastError();
+    }
     dim3 grid(m->nl.nitems, 2 * ((a.nvec + 127) / 128));
     if (prec == CHFSI_FP32) proj_kernel<float><<<grid, 128, 0, st>>>(m->nl, a);
     else proj_kernel<double><<<grid, 128, 0, st>>>(m->nl, a);
@@ -444,6 +580,19 @@ cudaError_t launch_proj(const chfsi_mesh* m, chfsi_prec prec, const ProjArgs& a,
 
 cudaError_t launch_back(const chfsi_mesh* m, chfsi_prec prec, const BackArgs& a, cudaStream_t st) {
     if (m->nl.nitems == 0) return cudaSuccess;
+    if (m->nl.uniform_np == 4 || m->nl.uniform_np == 8) {
+        dim3 grid(m->nl.nitems_big, 2 * ((a.nvec + 127) / 128));
+        const bool f32 = prec == CHFSI_FP32;
+        if (m->nl.uniform_np == 8) {
+            if (f32) back_fast_kernel<float, 8><<<grid, 128, 0, st>>>(m->nl, a);
+            else back_fast_kernel<double, 8><<<grid, 128, 0, st>>>(m->nl, a);
+        } else {
+            if (f32) back_fast_kernel<float, 4><<<grid, 128, 0, st>>>(m->nl, a);
+            else back_fast_kernel<double, 4><<<grid, 128, 0, st>>>(m->nl, a);
+        }
+        count_launch();
+        return cudaGetLastError();
+    }
     {
         dim3 gg(m->nl.natoms, 2 * m->nl.max_nproj, (a.nvec + 127) / 128);
         gmat_kernel<<<gg, 128, 0, st>>>(m->nl, reinterpret_cast<const double2*>(a.C),
