@@ -67,12 +67,18 @@ class GpuProblem:
         M2 = 2 * self.nnodes
         return A.reshape(M2, -1).conj().T @ (self.mass[:, None, None] * Bm).reshape(M2, -1)
 
-    def rayleigh_quotients(self, X):
-        HX = self.apply_MinvH(X)
-        mX = self.mass[:, None, None] * X
-        num = (mX.conj() * HX).sum(dim=(0, 1)).real
-        den = (mX.conj() * X).sum(dim=(0, 1)).real
-        return (num / den).cpu().numpy()
+    def rayleigh_quotients(self, X, block=32):
+        """x^H H x / x^H M x per column, in column blocks so that large multivectors need no full-size temporaries."""
+        out = []
+        for j0 in range(0, X.shape[-1], block):
+            Xb = X[:, :, j0:j0 + block].contiguous()
+            HX = self.apply_MinvH(Xb)
+            mX = self.mass[:, None, None] * Xb
+            num = (mX.conj() * HX).sum(dim=(0, 1)).real
+            den = (mX.conj() * Xb).sum(dim=(0, 1)).real
+            out.append((num / den).cpu().numpy())
+            del HX, mX
+        return np.concatenate(out)
 
     def lanczos_bounds(self, steps=10, seed=0):
         """(a0, b): lowest Ritz value and the safeguarded upper bound theta_max + ||f||_M."""
