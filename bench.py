@@ -34,6 +34,9 @@ from paper_2605_30128_b200 import inputs as inp  # noqa: E402
 METRIC = "chebyshev_filter_throughput"
 UNIT = "complex_DoF*vectors*degree/s"
 FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum per cell-kernel launch from the committed `ncu --set full`
+# captures (profiles/r1_final_ncu_full.md), keyed by (config, precision); None where no capture exists
+NCU_TRAFFIC = {(1, "fp64"): 2.031e9, (1, "fp32"): 2.030e9}
 
 
 def measured_hbm_peak():
@@ -119,7 +122,7 @@ def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    ncols = args.ref_cols
+    ncols = max(1, args.ref_cols // 4)      # each of the K + W steps is a bounded sample (~4 s): the run ends in about a minute
     times, cores = [], 1
     for i in range(args.warmup + args.steps):
         rate, dt, cores = cpu_oracle_rate(cfg, ncols)
@@ -217,7 +220,8 @@ def run_ours(args, cfg):
     achieved = cell_bytes / (cell_ms * 1e-3) / 1e9
     steps_prof = max(1, min(3, args.steps))
     roofline = {"bound": "hbm", "kernel": "cell_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src, "traffic": args.traffic,
+                "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": args.traffic if args.traffic is not None else (NCU_TRAFFIC.get((args.config, args.prec)) if nvec == cfg.nvec else None),
                 "avg_launch_ms": cell_ms / cell_n, "launches_per_step": cell_n // steps_prof,
                 "share_of_step": (cell_ms / steps_prof) / ms_step,
                 "alg_bytes_per_launch": cell_bytes / cell_n}
