@@ -139,7 +139,7 @@ struct MarchConsumer {
     static constexpr int NAH = (n - A0) < Cfg::NA ? (n - A0) : Cfg::NA;
     double acc[n][NAH];          // z-accumulators of the current cell: acc[k][ii], plane k, x-position A0 + ii
     double kyrow[n], wxy[NAH];
-    double wyj, pyj, fyj, cin, cR;
+    double wyj, pyj, fyj, cin, cR, sg;
     double* outcol;
     int j, col, s_spin, ri, ex, gy, g0;
     bool vok, jown, wy, xwrap, ywrap, valid;
@@ -149,6 +149,7 @@ struct MarchConsumer {
         valid = row < n;
         j = valid ? row : n - 1; col = col_; ex = ex_; g0 = g0_; xwrap = xw; ywrap = yw;
         s_spin = col / (C / 2); ri = col & 1;
+        sg = ((ri == 0) != (s_spin == 0)) ? -1.0 : 1.0;
         const int vl = (col % (C / 2)) >> 1;
         const int v = chunk * Cfg::NV + vl;
         vok = valid && v < ar.nvec;
@@ -292,16 +293,15 @@ struct MarchConsumer {
                 for (int ii = 0; ii < NAH; ++ii) {
                     const int a = A0 + ii;
                     if (a < P) {
+                        // (B_x -+ i B_y) u_other: real part B_x u_re +- B_y u_im, imaginary part B_x u_im -+ B_y u_re, i.e.
+                        // B_x * (other spin, same part) + sg * B_y * (other spin, other part), sg fixed per thread
                         const double in_own = row[a];
                         const double o_same = INc[Cfg::ofs(j, a) + ((col ^ (C / 2)) - col)];
                         const double o_flip = INc[Cfg::ofs(j, a) + ((col ^ (C / 2 + 1)) - col)];
-                        const double u_re = ri == 0 ? o_same : o_flip;       // other spin, same vector
-                        const double u_im = ri == 0 ? o_flip : o_same;
-                        const double4 f = *reinterpret_cast<const double4*>(Fs + (j * P + a) * 4);
-                        const double diag = s_spin == 0 ? f.x : f.y;
-                        const double sy = s_spin == 0 ? -f.w : f.w;
-                        const double offd = ri == 0 ? f.z * u_re - sy * u_im : f.z * u_im + sy * u_re;
-                        double val = fma(pz * sc.PX[a], fma(diag, in_own, offd), ip[ii]);
+                        const double diag = Fs[(j * P + a) * 4 + s_spin];
+                        const double2 bxy = *reinterpret_cast<const double2*>(Fs + (j * P + a) * 4 + 2);
+                        const double pot = fma(diag, in_own, fma(bxy.x, o_same, (sg * bxy.y) * o_flip));
+                        double val = fma(pz * sc.PX[a], pot, ip[ii]);
                         val = fma(fz * sc.FX[a], in_own, val);
                         if (ar.useR) val = fma(cR, Rs[(j * P + a) * C + col], val);
                         ip[ii] = val;
@@ -347,7 +347,7 @@ struct MarchConsumerF32 {
     float acc[n][NAH];
     float kyrow[n], wxy[NAH];
     float wyj;
-    double pyj, fyj, cin, cR;
+    double pyj, fyj, cin, cR, sg;
     double* outcol;
     double* pw;                  // PW + (j * P) * C + col : this thread's pointwise slots, [c][.][a][.]
     int j, col, s_spin, ri, ex, gy, g0;
@@ -358,6 +358,7 @@ struct MarchConsumerF32 {
         valid = row < n;
         j = valid ? row : n - 1; col = col_; ex = ex_; g0 = g0_; xwrap = xw; ywrap = yw;
         s_spin = col / (C / 2); ri = col & 1;
+        sg = ((ri == 0) != (s_spin == 0)) ? -1.0 : 1.0;
         const int vl = (col % (C / 2)) >> 1;
         const int v = chunk * Cfg::NV + vl;
         vok = valid && v < ar.nvec;
@@ -488,13 +489,9 @@ struct MarchConsumerF32 {
                         const double in_own = INc[Cfg::ofs(j, a)];
                         const double o_same = INc[Cfg::ofs(j, a) + ((col ^ (C / 2)) - col)];
                         const double o_flip = INc[Cfg::ofs(j, a) + ((col ^ (C / 2 + 1)) - col)];
-                        const double u_re = ri == 0 ? o_same : o_flip;
-                        const double u_im = ri == 0 ? o_flip : o_same;
-                        const double4 fl = *reinterpret_cast<const double4*>(Fs + (j * P + a) * 4);
-                        const double diag = s_spin == 0 ? fl.x : fl.y;
-                        const double sy = s_spin == 0 ? -fl.w : fl.w;
-                        const double offd = ri == 0 ? fl.z * u_re - sy * u_im : fl.z * u_im + sy * u_re;
-                        double val = (pz * sc.PX[a]) * fma(diag, in_own, offd);
+                        const double diag = Fs[(j * P + a) * 4 + s_spin];
+                        const double2 bxy = *reinterpret_cast<const double2*>(Fs + (j * P + a) * 4 + 2);
+                        double val = (pz * sc.PX[a]) * fma(diag, in_own, fma(bxy.x, o_same, (sg * bxy.y) * o_flip));
                         val = fma(fz * sc.FX[a], in_own, val);
                         if (ar.useR) val = fma(cR, Rs[(j * P + a) * C + col], val);
                         pwc[a * C] = val;
