@@ -140,6 +140,7 @@ struct MarchConsumer {
     double acc[n][NAH];          // z-accumulators of the current cell: acc[k][ii], plane k, x-position A0 + ii
     double kyrow[n], wxy[NAH];
     double wyj, pyj, fyj, cin, cR, sg;
+    double pAr, pAi, pBr, pBi;   // Bloch phase of this row's plain and x-face entries (HASPH)
     double* outcol;
     int j, col, s_spin, ri, ex, gy, g0;
     bool vok, jown, wy, xwrap, ywrap, valid;
@@ -162,6 +163,10 @@ struct MarchConsumer {
         cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
         cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
         gy = ey * P + j; wy = gy == ar.n1[1]; if (wy) gy = 0;
+        pAr = 1.0; pAi = 0.0;
+        if (HASPH && wy) { pAr = ar.ph_re[1]; pAi = ar.ph_im[1]; }
+        pBr = pAr; pBi = pAi;
+        if (HASPH && xwrap) { pBr = pAr * ar.ph_re[0] - pAi * ar.ph_im[0]; pBi = pAr * ar.ph_im[0] + pAi * ar.ph_re[0]; }
         outcol = ar.out + ((long long)s_spin * ar.ld_out + (vok ? v : 0)) * 2 + ri;
 #pragma unroll
         for (int k = 0; k < n; ++k)
@@ -186,6 +191,17 @@ struct MarchConsumer {
         for (int k = 0; k < n; ++k) {
             if (k < nk) {
                 int gz = gzbase + k; const bool wz = gz == ar.n1[2]; if (wz) gz = 0;
+                const bool anyw = xwrap | ywrap | wz;                  // CTA-uniform: interior CTAs skip the phase arithmetic
+                double ar_ = pAr, ai_ = pAi, br_ = pBr, bi_ = pBi;      // conj-phase of plain / x-face columns of this row
+                if (HASPH) {
+                    if (wz) {
+                        const double zr_ = ar.ph_re[2], zi_ = ar.ph_im[2];
+                        const double t0 = ar_ * zr_ - ai_ * zi_; ai_ = ar_ * zi_ + ai_ * zr_; ar_ = t0;
+                        const double t1 = br_ * zr_ - bi_ * zi_; bi_ = br_ * zi_ + bi_ * zr_; br_ = t1;
+                    }
+                    if (ri) { ai_ = -ai_; bi_ = -bi_; }
+                }
+                (void)ar_; (void)ai_; (void)br_; (void)bi_; (void)anyw;
                 double* line = outcol + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xstride;
                 double* pnode = line + x0 * xstride;
 #pragma unroll
@@ -193,12 +209,11 @@ struct MarchConsumer {
                     const bool wx = (A0 + ii == P) && xwrap;
                     double* dst = wx ? line : pnode + ii * xstride;
                     double val = acc[k][ii];
-                    if (HASPH) {
+                    if (HASPH && anyw) {
+                        // times conj(phase), branch-free: (pr, pi) is (1, 0) where nothing wrapped
                         const double other = __shfl_xor_sync(0xffffffffu, val, 1);
-                        if (wx | wy | wz) {
-                            double pr, pi; phase_of(ar, wx, wy, wz, pr, pi);
-                            val = ri == 0 ? val * pr + other * pi : val * pr - other * pi;   // times conj(phase)
-                        }
+                        const bool fc = A0 + ii == P;
+                        val = fma(other, fc ? bi_ : ai_, val * (fc ? br_ : ar_));
                     }
                     if (vok) atomicAdd(dst, val);
                 }
@@ -565,6 +580,7 @@ struct MarchConsumerF32 {
     float kyrow[n], wxy[NAH];
     float wyj;
     double pyj, fyj, cin, cR, sg;
+    double pAr, pAi, pBr, pBi;
     double* outcol;
     double* pw;                  // PW + (j * P) * C + col : this thread's pointwise slots, [c][.][a][.]
     int j, col, s_spin, ri, ex, gy, g0;
@@ -588,6 +604,10 @@ struct MarchConsumerF32 {
         cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
         cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
         gy = ey * P + j; wy = gy == ar.n1[1]; if (wy) gy = 0;
+        pAr = 1.0; pAi = 0.0;
+        if (HASPH && wy) { pAr = ar.ph_re[1]; pAi = ar.ph_im[1]; }
+        pBr = pAr; pBi = pAi;
+        if (HASPH && xwrap) { pBr = pAr * ar.ph_re[0] - pAi * ar.ph_im[0]; pBi = pAr * ar.ph_im[0] + pAi * ar.ph_re[0]; }
         outcol = ar.out + ((long long)s_spin * ar.ld_out + (vok ? v : 0)) * 2 + ri;
         pw = PW + (jown ? j : 0) * P * C + col;
 #pragma unroll
@@ -611,6 +631,17 @@ struct MarchConsumerF32 {
         for (int k = 0; k < n; ++k) {
             if (k < nk) {
                 int gz = gzbase + k; const bool wz = gz == ar.n1[2]; if (wz) gz = 0;
+                const bool anyw = xwrap | ywrap | wz;                  // CTA-uniform: interior CTAs skip the phase arithmetic
+                double ar_ = pAr, ai_ = pAi, br_ = pBr, bi_ = pBi;      // conj-phase of plain / x-face columns of this row
+                if (HASPH) {
+                    if (wz) {
+                        const double zr_ = ar.ph_re[2], zi_ = ar.ph_im[2];
+                        const double t0 = ar_ * zr_ - ai_ * zi_; ai_ = ar_ * zi_ + ai_ * zr_; ar_ = t0;
+                        const double t1 = br_ * zr_ - bi_ * zi_; bi_ = br_ * zi_ + bi_ * zr_; br_ = t1;
+                    }
+                    if (ri) { ai_ = -ai_; bi_ = -bi_; }
+                }
+                (void)ar_; (void)ai_; (void)br_; (void)bi_; (void)anyw;
                 double* line = outcol + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xstride;
                 double* pnode = line + x0 * xstride;
 #pragma unroll
@@ -621,12 +652,11 @@ struct MarchConsumerF32 {
                     if (A0 + ii < P && k < P) {
                         if (with_pw && jown) val += pw[(k * P * P + A0 + ii) * C];
                     }
-                    if (HASPH) {
+                    if (HASPH && anyw) {
+                        // times conj(phase), branch-free: (pr, pi) is (1, 0) where nothing wrapped
                         const double other = __shfl_xor_sync(0xffffffffu, val, 1);
-                        if (wx | wy | wz) {
-                            double pr, pi; phase_of(ar, wx, wy, wz, pr, pi);
-                            val = ri == 0 ? val * pr + other * pi : val * pr - other * pi;   // times conj(phase)
-                        }
+                        const bool fc = A0 + ii == P;
+                        val = fma(other, fc ? bi_ : ai_, val * (fc ? br_ : ar_));
                     }
                     if (vok) atomicAdd(dst, val);
                 }
