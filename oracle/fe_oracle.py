@@ -169,6 +169,8 @@ class Mesh:
         for e in range(ncells):
             np.add.at(m, self.cell_nodes[e], self.wq)
         self.mass = m
+        # with a single cell in some direction a cell lists a global node twice (its two faces coincide)
+        self.cell_unique = min(self.ncell) > 1
 
     def node_coords(self) -> np.ndarray:
         """[M,3] coordinates, node I = (iz N1y + iy) N1x + ix, x = (e + (xi+1)/2) h."""
@@ -269,7 +271,10 @@ def apply_H(ham: Hamiltonian, X: np.ndarray, use_dense_cell=False) -> np.ndarray
         Ye = np.empty_like(Xe)
         Ye[:, 0, :] = 0.5 * KX[:, 0, :] + (wV + wBz) * up + (wBx - 1j * wBy) * dn     # (ii)
         Ye[:, 1, :] = 0.5 * KX[:, 1, :] + (wBx + 1j * wBy) * up + (wV - wBz) * dn
-        Y[idx] += np.conj(ph)[:, None, None] * Ye                   # (iii) idx unique within a cell
+        if mesh.cell_unique:                                         # (iii) scatter-ADD
+            Y[idx] += np.conj(ph)[:, None, None] * Ye
+        else:                                                        # a direction with one cell: both faces are the
+            np.add.at(Y, idx, np.conj(ph)[:, None, None] * Ye)      # same global node, contributions accumulate
     for nodes, Pa, Da in ham.atoms:                                  # (iv)
         npj = Pa.shape[1]
         mX = mesh.mass[nodes][:, None, None] * X[nodes]              # [ns,2,nvec]

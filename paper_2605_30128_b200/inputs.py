@@ -22,7 +22,8 @@ import numpy as np
 
 @dataclasses.dataclass(frozen=True)
 class Config:
-    """One BASELINE.json workload.  `ncell` cells per direction on a cube of side `L` Bohr."""
+    """One BASELINE.json workload.  `ncell` cells per direction on a cube of side `L` Bohr
+    (scalars; test meshes may pass 3-tuples for a box with different cell counts / sides per direction)."""
     name: str
     ncell: int
     L: float
@@ -37,12 +38,21 @@ class Config:
     ngauss: int = 0       # >0: that many seeded Gaussian wells (config 0); 0: one per atom
 
     @property
+    def ncell3(self):
+        return (self.ncell,) * 3 if np.ndim(self.ncell) == 0 else tuple(self.ncell)
+
+    @property
+    def L3(self) -> np.ndarray:
+        return np.full(3, float(self.L)) if np.ndim(self.L) == 0 else np.asarray(self.L, dtype=np.float64)
+
+    @property
     def n1(self) -> int:
         return self.ncell * self.p
 
     @property
     def nnodes(self) -> int:
-        return self.n1 ** 3
+        nc = self.ncell3
+        return nc[0] * nc[1] * nc[2] * self.p ** 3
 
 
 CONFIGS = {
@@ -89,10 +99,12 @@ def atom_positions(cfg: Config, seed: int = 0) -> np.ndarray:
     """[natoms,3] positions in [0,L)^3.  Config 0: seeded uniform; else jittered lattice."""
     rng = np.random.default_rng([seed, 101])
     if cfg.ngauss > 0:                       # config-0 style: free seeded positions
-        return rng.uniform(0.0, cfg.L, size=(cfg.natoms, 3))
+        return rng.uniform(0.0, 1.0, size=(cfg.natoms, 3)) * cfg.L3[None, :]
     na = round(cfg.natoms ** (1.0 / 3.0))
     if na ** 3 != cfg.natoms:
         raise ValueError("jittered lattice needs a cubic atom count")
+    if np.ndim(cfg.L) != 0:
+        raise ValueError("jittered lattice is defined for cubic boxes")
     a = cfg.L / na
     g = (np.arange(na) + 0.5) * a
     zz, yy, xx = np.meshgrid(g, g, g, indexing="ij")
@@ -104,12 +116,12 @@ def atom_positions(cfg: Config, seed: int = 0) -> np.ndarray:
 def gaussian_centres(cfg: Config, atoms: np.ndarray, seed: int = 0) -> np.ndarray:
     if cfg.ngauss > 0:
         rng = np.random.default_rng([seed, 102])
-        return rng.uniform(0.0, cfg.L, size=(cfg.ngauss, 3))
+        return rng.uniform(0.0, 1.0, size=(cfg.ngauss, 3)) * cfg.L3[None, :]
     return atoms.copy()
 
 
-def _min_image(d: np.ndarray, L: float):
-    """Minimum-image displacement and the integer lattice shift n with d_min = d + n*L."""
+def _min_image(d: np.ndarray, L):
+    """Minimum-image displacement and the integer lattice shift n with d_min = d + n*L (L scalar or per column)."""
     n = -np.rint(d / L)
     return d + n * L, n
 
@@ -144,26 +156,27 @@ def local_fields(cfg: Config, xyz: np.ndarray, centres: np.ndarray):
     axes = _tensor_axes(xyz)
     if axes is not None:
         ux, uy, uz = axes
-        img = np.array([-1.0, 0.0, 1.0]) * cfg.L
+        L3 = cfg.L3
 
-        def g1(u, c):
-            d = u[:, None] - c - img[None, :]
+        def g1(u, c, Ld):
+            d = u[:, None] - c - np.array([-1.0, 0.0, 1.0])[None, :] * Ld
             return np.exp(-d * d / (2.0 * V_WIDTH ** 2)).sum(axis=1)
 
         V3 = np.zeros((uz.size, uy.size, ux.size))
         for c in centres:
-            V3 += V_DEPTH * g1(uz, c[2])[:, None, None] * g1(uy, c[1])[None, :, None] * g1(ux, c[0])[None, None, :]
+            V3 += (V_DEPTH * g1(uz, c[2], L3[2])[:, None, None] * g1(uy, c[1], L3[1])[None, :, None]
+                   * g1(ux, c[0], L3[0])[None, None, :])
         V = V3.reshape(M)
     else:
         shifts = np.array([(i, j, k) for i in (-1, 0, 1) for j in (-1, 0, 1) for k in (-1, 0, 1)],
-                          dtype=np.float64) * cfg.L
+                          dtype=np.float64) * cfg.L3[None, :]
         for c in centres:
             d0 = xyz - c[None, :]
             for s in shifts:
                 d = d0 - s[None, :]
                 r2 = np.einsum("ij,ij->i", d, d)
                 V += V_DEPTH * np.exp(-r2 / (2.0 * V_WIDTH ** 2))
-    ang = 2.0 * math.pi * xyz[:, 0] / cfg.L
+    ang = 2.0 * math.pi * xyz[:, 0] / cfg.L3[0]
     Bx = np.zeros(M)
     By = B_MAG * np.cos(ang)
     Bz = B_MAG * np.sin(ang)
@@ -180,7 +193,7 @@ def projector_tables(cfg: Config, xyz: np.ndarray, atoms: np.ndarray, cutoff: fl
     minimum image; shapes: exp(-r^2/2 sigma^2) x {1, x, y, z},
     analytically normalised over all space, hard cutoff at `cutoff`.
     """
-    L = cfg.L
+    L = cfg.L3
     kfrac = np.asarray(cfg.kfrac, dtype=np.float64)
     supp_off = [0]
     supp_nodes = []
@@ -192,17 +205,17 @@ def projector_tables(cfg: Config, xyz: np.ndarray, atoms: np.ndarray, cutoff: fl
             # candidate nodes: the per-axis index ranges within the cutoff (same per-node arithmetic as below)
             sel = []
             for ax in range(3):
-                d1, _ = _min_image(axes[ax] - Ra[ax], L)
+                d1, _ = _min_image(axes[ax] - Ra[ax], L[ax])
                 sel.append(np.nonzero(np.abs(d1) < cutoff)[0])
             nx, ny = axes[0].size, axes[1].size
             cand = ((sel[2][:, None, None] * ny + sel[1][None, :, None]) * nx + sel[0][None, None, :]).reshape(-1)
-            d, n = _min_image(xyz[cand] - Ra[None, :], L)
+            d, n = _min_image(xyz[cand] - Ra[None, :], L[None, :])
             r2 = np.einsum("ij,ij->i", d, d)
             keep = np.nonzero(r2 < cutoff ** 2)[0]
             idx = cand[keep]
             dd, nn, rr2 = d[keep], n[keep], r2[keep]
         else:
-            d, n = _min_image(xyz - Ra[None, :], L)
+            d, n = _min_image(xyz - Ra[None, :], L[None, :])
             r2 = np.einsum("ij,ij->i", d, d)
             idx = np.nonzero(r2 < cutoff ** 2)[0]
             dd, nn, rr2 = d[idx], n[idx], r2[idx]

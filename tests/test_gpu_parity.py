@@ -34,7 +34,7 @@ class Problem:
         xyz = self.omesh.node_coords()
         assert B.chfsi_mesh_num_nodes(self.gmesh) == self.omesh.nnodes
         gx = B.chfsi_mesh_node_coords(self.gmesh)
-        assert np.max(np.abs(gx - xyz)) < 1e-13 * cfg.L
+        assert np.max(np.abs(gx - xyz)) < 1e-13 * float(np.max(cfg.L))
         gm = B.chfsi_mesh_mass(self.gmesh)
         assert np.max(np.abs(gm - self.omesh.mass)) < 1e-13 * np.max(gm)
         hi = inp.make_hamiltonian(cfg, xyz, seed=seed, with_local=with_local, with_nonlocal=with_nonlocal)
@@ -177,6 +177,60 @@ def test_filter_chunked_equals_unchunked_and_ragged(env):
         assert relerr(full, ref) < TOL64 and relerr(chunked, ref) < TOL64
         ch10 = pb.gpu_filter(X, None, 7, a, b, a0, B.FP64, B.RECUR_STANDARD, chunk=8)
         assert relerr(ch10, ref) < TOL64
+    finally:
+        pb.close()
+
+
+# ------------------------------------------------------------------------------- boxes that are not cubes
+@pytest.mark.parametrize("p,ncell,L,kfrac", [(4, (2, 3, 4), (3.0, 4.5, 5.0), (0.25, -0.1, 0.4)),
+                                             (6, (3, 1, 2), (6.0, 2.5, 4.0), (0, 0, 0)),
+                                             (8, (1, 2, 3), (2.5, 4.0, 6.5), (0, 0.5, 0.125)),
+                                             (6, (1, 1, 1), (3.0, 3.0, 3.0), (0.3, 0.3, 0.3)),
+                                             (3, (2, 4, 3), (4.0, 7.0, 6.0), (0, 0, 0.2))])
+def test_anisotropic_box_apply_and_filter(env, p, ncell, L, kfrac):
+    """Different cell counts and side lengths per direction (a single cell per direction included: every face then
+    wraps onto the cell itself), with Bloch phases; operator and both recurrences, FP64 and FP32 product."""
+    _, fo, B = env
+    cfg = inp.tiny_config(ncell=ncell, p=p, L=L, kfrac=kfrac, nvec=7, natoms=2, nproj=8, ngauss=3)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, 7)
+        ref = fo.apply_MinvH(pb.oham, X)
+        assert relerr(pb.gpu_apply(X, B.FP64), ref) < 1e-13
+        assert relerr(pb.gpu_apply(X, B.FP32), ref) < 2e-6
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref11 = fo.cheb_filter_residual(pb.oham, X, lam, 9, a, b, a0)
+        assert relerr(pb.gpu_filter(X, lam, 9, a, b, a0, B.FP64, B.RECUR_RESIDUAL), ref11) < TOL64
+        assert relerr(pb.gpu_filter(X, None, 9, a, b, a0, B.FP64, B.RECUR_STANDARD), ref11) < TOL64
+        assert relerr(pb.gpu_filter(X, lam, 9, a, b, a0, B.FP32, B.RECUR_RESIDUAL), ref11) < TOL32
+    finally:
+        pb.close()
+
+
+def test_single_vector_and_wide_leading_dimension_in_filter(env):
+    """nvec = 1 (one lane pair of one CTA active) and a filter call on a column window of a wider block (ld > nvec)."""
+    torch, fo, B = env
+    cfg = inp.tiny_config(ncell=2, p=6, L=4.0, kfrac=(0.25, 0, 0), nvec=13, natoms=1, nproj=8, ngauss=2)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, 13)
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref = fo.cheb_filter_residual(pb.oham, X, lam, 6, a, b, a0)
+        one = pb.gpu_filter(X[:, :, :1].copy(), lam[:1], 6, a, b, a0, B.FP64, B.RECUR_RESIDUAL)
+        assert relerr(one, ref[:, :, :1]) < TOL64
+        # columns 2..10 of a 13-wide device block, output into a 16-wide block; the rest must stay untouched
+        Xd = torch.from_numpy(X).cuda()
+        Yd = torch.full((cfg.nnodes, 2, 16), 5.0, dtype=torch.complex128, device="cuda")
+        for prec, tol in [(B.FP64, TOL64), (B.FP32, TOL32)]:
+            Yd.fill_(5.0)
+            B.chfsi_cheb_filter(pb.gmesh, prec, B.RECUR_RESIDUAL, 6, a, b, a0, Xd[:, :, 2:11], lam[2:11], Yd[:, :, 3:12],
+                                pb.work(prec, B.RECUR_RESIDUAL, 9), nvec=9, ldx=13, ldy=16)
+            torch.cuda.synchronize()
+            Y = Yd.cpu().numpy()
+            assert relerr(Y[:, :, 3:12], ref[:, :, 2:11]) < tol
+            assert np.all(Y[:, :, :3] == 5.0) and np.all(Y[:, :, 12:] == 5.0)
     finally:
         pb.close()
 

@@ -125,10 +125,13 @@ def test_p3_hermiticity_all_terms(kfrac):
 
 
 # ------------------------------------------------------------------ P4
+@pytest.mark.parametrize("nc", [(2, 3, 2), (1, 3, 2), (2, 1, 1), (1, 1, 1)])
 @pytest.mark.parametrize("kfrac", [(0.0, 0.0, 0.0), (0.25, 0.1, 0.0)])
-def test_p4_kronecker_line_operator_form(kfrac):
-    """M^-1 K = A_x (x) I (x) I + I (x) A_y (x) I + I (x) I (x) A_z, A_d = M1^-1 K1 assembled in 1-D."""
-    nc, L, p = (2, 3, 2), (2.0, 3.3, 1.7), 3
+def test_p4_kronecker_line_operator_form(kfrac, nc):
+    """M^-1 K = A_x (x) I (x) I + I (x) A_y (x) I + I (x) I (x) A_z, A_d = M1^-1 K1 assembled in 1-D.
+    Single-cell directions included: there a cell's two faces are the same global node, so the assembly
+    (PAPER.md:204 (iii)) has to accumulate both local contributions."""
+    L, p = (2.0, 3.3, 1.7), 3
     mesh = fo.Mesh(nc, L, p, kfrac)
     ham = fo.Hamiltonian(mesh, None, None, None, None)
     X = inp.make_vectors(mesh.nnodes, 3, seed=2)
