@@ -272,6 +272,9 @@ def _sampled_config_case(env, cfg, cols, precs, nvec_gpu, chunk=0):
             Y = pb.gpu_filter(X, lam, cfg.degree, a, b, a0, prec, B.RECUR_RESIDUAL, chunk=chunk)
             out[prec] = relerr(Y[:, :, cols], ref)
             assert out[prec] < tol, (prec, out[prec])
+        # eq. 10 (three-term recurrence) at full size: same polynomial (P5), so the same reference
+        Y10 = pb.gpu_filter(X, None, cfg.degree, a, b, a0, B.FP64, B.RECUR_STANDARD, chunk=chunk)
+        assert relerr(Y10[:, :, cols], ref) < TOL64
         return out
     finally:
         pb.close()
