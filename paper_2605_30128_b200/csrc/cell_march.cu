@@ -126,7 +126,8 @@ struct MarchCfg {
     static constexpr int PW_BYTES = P * P * P * C * 8;
     static constexpr int STAGES32_ = (200 * 1024 - PW_BYTES - NFB * FB_BYTES) / STAGE_BYTES;
     static constexpr int STAGES32 = STAGES32_ < 8 ? STAGES32_ : 8;
-    static constexpr int NCW = 4;                         // converter warps
+    // converter warps: fill the CTA up to whole groups of four warps (one per scheduler)
+    static constexpr int NCW = 4 - (CWARPS + 1) % 4;
     static constexpr int THREADS32 = (CWARPS + 1 + NCW) * 32;
 };
 
@@ -1051,7 +1052,7 @@ cudaError_t launch_cell_march(const chfsi_mesh* m, chfsi_prec prec, const CellAr
         case 2: return f32 ? launch_march_t<2, 32, 1, true>(m, a, st) : launch_march_t<2, 32, 1, false>(m, a, st);
         case 4: return f32 ? launch_march_t<4, 32, 1, true>(m, a, st) : launch_march_t<4, 32, 1, false>(m, a, st);
         case 6: return f32 ? launch_march_t<6, 32, 1, true>(m, a, st) : launch_march_t<6, 32, 1, false>(m, a, st);
-        case 8: return f32 ? launch_march_t<8, 16, 3, true>(m, a, st) : launch_march_t<8, 16, 3, false>(m, a, st);
+        case 8: return f32 ? launch_march_t<8, 16, 1, true>(m, a, st) : launch_march_t<8, 16, 3, false>(m, a, st);
         default: return cudaErrorInvalidValue;
     }
 }
