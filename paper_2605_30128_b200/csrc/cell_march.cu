@@ -139,7 +139,6 @@ struct MarchConsumer {
     static constexpr int A0 = H * Cfg::NA;
     static constexpr int NAH = (n - A0) < Cfg::NA ? (n - A0) : Cfg::NA;
     double acc[n][NAH];          // z-accumulators of the current cell: acc[k][ii], plane k, x-position A0 + ii
-    double kyrow[n], wxy[NAH];
     double wyj, pyj, fyj, cin, cR, sg;
     double pAr, pAi, pBr, pBi;   // Bloch phase of this row's plain and x-face entries (HASPH)
     double* outcol;
@@ -156,10 +155,6 @@ struct MarchConsumer {
         const int v = chunk * Cfg::NV + vl;
         vok = valid && v < ar.nvec;
         jown = j < P;
-#pragma unroll
-        for (int b = 0; b < n; ++b) kyrow[b] = sc.KY[j][b];
-#pragma unroll
-        for (int ii = 0; ii < NAH; ++ii) wxy[ii] = sc.WX[A0 + ii] * sc.WY[j];
         wyj = sc.WY[j]; pyj = sc.PY[j]; fyj = sc.FY[j];
         cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
         cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
@@ -261,7 +256,7 @@ struct MarchConsumer {
         for (int ii = 0; ii < NAH; ++ii) {
             double sy = 0.0;
 #pragma unroll
-            for (int b = 0; b < n; ++b) sy = fma(kyrow[b], INc[Cfg::ofs(b, A0 + ii)], sy);
+            for (int b = 0; b < n; ++b) sy = fma(sc.KY[j][b], INc[Cfg::ofs(b, A0 + ii)], sy);
             ip[ii] = sc.WX[A0 + ii] * sy;
         }
         // x-contraction on the own row, own outputs
@@ -274,7 +269,7 @@ struct MarchConsumer {
         }
         double zr[NAH];
 #pragma unroll
-        for (int ii = 0; ii < NAH; ++ii) zr[ii] = wxy[ii] * row[A0 + ii];
+        for (int ii = 0; ii < NAH; ++ii) zr[ii] = sc.WX[A0 + ii] * (wyj * row[A0 + ii]);
         if (lower) {
 #pragma unroll
             for (int k = 0; k < n; ++k)
