@@ -139,7 +139,7 @@ struct MarchConsumer {
     static constexpr int A0 = H * Cfg::NA;
     static constexpr int NAH = (n - A0) < Cfg::NA ? (n - A0) : Cfg::NA;
     double acc[n][NAH];          // z-accumulators of the current cell: acc[k][ii], plane k, x-position A0 + ii
-    double wyj, pyj, fyj, cin, cR, sg;
+    double cin, cR, sg;          // W_y[j], P_y[j], F_y[j] are re-fetched from the constant bank where used
     double pAr, pAi, pBr, pBi;   // Bloch phase of this row's plain and x-face entries (HASPH)
     double* outcol;
     int j, col, s_spin, ri, ex, gy, g0;
@@ -155,7 +155,6 @@ struct MarchConsumer {
         const int v = chunk * Cfg::NV + vl;
         vok = valid && v < ar.nvec;
         jown = j < P;
-        wyj = sc.WY[j]; pyj = sc.PY[j]; fyj = sc.FY[j];
         cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
         cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
         gy = ey * P + j; wy = gy == ar.n1[1]; if (wy) gy = 0;
@@ -265,11 +264,11 @@ struct MarchConsumer {
             double sx = 0.0;
 #pragma unroll
             for (int a = 0; a < n; ++a) sx = fma(sc.KX[A0 + ii][a], row[a], sx);
-            ip[ii] = fma(wyj, sx, ip[ii]);
+            ip[ii] = fma(sc.WY[j], sx, ip[ii]);
         }
         double zr[NAH];
 #pragma unroll
-        for (int ii = 0; ii < NAH; ++ii) zr[ii] = sc.WX[A0 + ii] * (wyj * row[A0 + ii]);
+        for (int ii = 0; ii < NAH; ++ii) zr[ii] = sc.WX[A0 + ii] * (sc.WY[j] * row[A0 + ii]);
         if (lower) {
 #pragma unroll
             for (int k = 0; k < n; ++k)
@@ -299,7 +298,7 @@ struct MarchConsumer {
             for (int ii = 0; ii < NAH; ++ii) ip[ii] *= wzc;
             if (jown) {
                 // S5 on the owned nodes of this plane (a < P): eq. 12 spin blocks, in-term, R-term
-                const double pz = sc.PZ[c] * pyj, fz = sc.FZ[c] * fyj * cin;
+                const double pz = sc.PZ[c] * sc.PY[j], fz = sc.FZ[c] * sc.FY[j] * cin;
 #pragma unroll
                 for (int ii = 0; ii < NAH; ++ii) {
                     const int a = A0 + ii;
