@@ -1046,7 +1046,7 @@ cudaError_t launch_cell_march(const chfsi_mesh* m, chfsi_prec prec, const CellAr
         case 2: return f32 ? launch_march_t<2, 32, 1, true>(m, a, st) : launch_march_t<2, 32, 1, false>(m, a, st);
         case 4: return f32 ? launch_march_t<4, 32, 1, true>(m, a, st) : launch_march_t<4, 32, 1, false>(m, a, st);
         case 6: return f32 ? launch_march_t<6, 32, 1, true>(m, a, st) : launch_march_t<6, 32, 1, false>(m, a, st);
-        case 8: return f32 ? launch_march_t<8, 16, 1, true>(m, a, st) : launch_march_t<8, 16, 3, false>(m, a, st);
+        case 8: return f32 ? launch_march_t<8, 16, 1, true>(m, a, st) : launch_march_t<8, 16, 2, false>(m, a, st);
         default: return cudaErrorInvalidValue;
     }
 }
