@@ -344,223 +344,6 @@ struct MarchConsumer {
 };
 
 // ---------------------------------------------------------------------------------------------
-// Uniform-code consumer for even splits ((p+1) % XS == 0, e.g. p = 8: three parts of 3 x-positions).  All parts run
-// the SAME instructions: the part index is a runtime value that shifts the shared-memory base pointer and the row of
-// K_x fetched from the constant bank (LDC with a register index); only the x = P face column of the last part, which
-// lives in the FACE block of the stage, takes a warp-uniform branch.  One copy of the code instead of XS keeps the
-// kernel inside the instruction cache (the per-part instantiation of p = 8 was 122 KB of SASS and spent 42 % of its
-// issue slots on `no_instruction`).
-template <int P, int CC, int XSPLIT, bool HASPH>
-struct MarchConsumerU {
-    using Cfg = MarchCfg<P, CC, XSPLIT>;
-    static constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES, NA = Cfg::NA;
-    double acc[n][NA];
-    double wxy[NA], wxv[NA];     // K_y row j, P_x, F_x are re-fetched from the constant bank (register budget: 128)
-    double wyj, pyj, fyj, cin, cR, sg;
-    double* outcol;
-    int j, col, s_spin, ri, ex, gy, g0, a0;
-    bool vok, jown, wy, xwrap, ywrap, valid, isface;
-
-    __device__ __forceinline__ void init(const StepConst& sc, const MarchArgs& ar, int h, int row, int col_, int ex_, int ey,
-                                         int chunk, int g0_, bool xw, bool yw) {
-        valid = row < n;
-        j = valid ? row : n - 1; col = col_; ex = ex_; g0 = g0_; xwrap = xw; ywrap = yw;
-        a0 = h * NA; isface = (a0 + NA - 1) == P;
-        s_spin = col / (C / 2); ri = col & 1;
-        sg = ((ri == 0) != (s_spin == 0)) ? -1.0 : 1.0;
-        const int vl = (col % (C / 2)) >> 1;
-        const int v = chunk * Cfg::NV + vl;
-        vok = valid && v < ar.nvec;
-        jown = j < P;
-#pragma unroll
-        for (int ii = 0; ii < NA; ++ii) {
-            wxv[ii] = sc.WX[a0 + ii]; wxy[ii] = wxv[ii] * sc.WY[j];
-        }
-        wyj = sc.WY[j]; pyj = sc.PY[j]; fyj = sc.FY[j];
-        cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
-        cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
-        gy = ey * P + j; wy = gy == ar.n1[1]; if (wy) gy = 0;
-        outcol = ar.out + ((long long)s_spin * ar.ld_out + (vok ? v : 0)) * 2 + ri;
-#pragma unroll
-        for (int k = 0; k < n; ++k)
-#pragma unroll
-            for (int ii = 0; ii < NA; ++ii) acc[k][ii] = 0.0;
-    }
-
-    __device__ __forceinline__ static void phase_of(const MarchArgs& ar, bool wx, bool wyy, bool wz, double& pr, double& pi) {
-        pr = 1.0; pi = 0.0;
-        if (wx) { pr = ar.ph_re[0]; pi = ar.ph_im[0]; }
-        if (wyy) { const double tt = pr * ar.ph_re[1] - pi * ar.ph_im[1]; pi = pr * ar.ph_im[1] + pi * ar.ph_re[1]; pr = tt; }
-        if (wz) { const double tt = pr * ar.ph_re[2] - pi * ar.ph_im[2]; pi = pr * ar.ph_im[2] + pi * ar.ph_re[2]; pr = tt; }
-    }
-
-    // shared-memory offset (doubles, without the lane's column) of entry (row b, own column ii) of a stage
-    __device__ __forceinline__ int eofs(int b, int ii) const {
-        return (isface && ii == NA - 1) ? (n * P + b) * C : (b * P + a0 + ii) * C;
-    }
-
-    __device__ __forceinline__ void emit(const MarchArgs& ar, int gzbase, int nk) {
-        const long long xstride = 4 * ar.ld_out;
-        const long long x0 = (long long)ex * P + a0;
-#pragma unroll
-        for (int k = 0; k < n; ++k) {
-            if (k < nk) {
-                int gz = gzbase + k; const bool wz = gz == ar.n1[2]; if (wz) gz = 0;
-                double* line = outcol + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xstride;
-                double* pnode = line + x0 * xstride;
-#pragma unroll
-                for (int ii = 0; ii < NA; ++ii) {
-                    const bool wx = (ii == NA - 1) && isface && xwrap;
-                    double* dst = wx ? line : pnode + ii * xstride;
-                    double val = acc[k][ii];
-                    if (HASPH) {
-                        const double other = __shfl_xor_sync(0xffffffffu, val, 1);
-                        if (wx | wy | wz) {
-                            double pr, pi; phase_of(ar, wx, wy, wz, pr, pi);
-                            val = ri == 0 ? val * pr + other * pi : val * pr - other * pi;   // times conj(phase)
-                        }
-                    }
-                    if (vok) atomicAdd(dst, val);
-                }
-            }
-        }
-    }
-
-    __device__ __forceinline__ void plane(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, uint64_t* full_bar,
-                                          uint64_t* empty_bar, int t, int c, bool lower, bool upper) {
-        const int s = t % STAGES;
-        const uint32_t par = (t / STAGES) & 1;
-        mbar_wait(&full_bar[s], par);
-        double* IN = reinterpret_cast<double*>(smem + (size_t)s * Cfg::STAGE_BYTES);
-        const double* Rs = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES + Cfg::R_OFF);
-        const double* Fs = reinterpret_cast<const double*>(smem + (size_t)s * Cfg::STAGE_BYTES + Cfg::F_OFF);
-        if (HASPH) {
-            const bool wz = (g0 + t) == ar.n1[2];
-            if (xwrap | ywrap | wz) {                                    // CTA-uniform
-                const bool wyy = ywrap && j == P;
-#pragma unroll
-                for (int ii = 0; ii < NA; ++ii) {
-                    const bool wx = xwrap && isface && (ii == NA - 1);
-                    const int o = eofs(j, ii) + col;
-                    const double val = IN[o];
-                    const double other = __shfl_xor_sync(0xffffffffu, val, 1);
-                    if ((wx | wyy | wz) && valid) {
-                        double pr, pi; phase_of(ar, wx, wyy, wz, pr, pi);
-                        IN[o] = ri == 0 ? val * pr - other * pi : other * pi + val * pr;
-                    }
-                }
-                asm volatile("bar.sync 1, %0;" ::"r"(Cfg::CWARPS * 32) : "memory");   // consumer warps only
-            }
-        }
-        const double* INc = IN + col;
-        const double* base = INc + a0 * C;                       // column a0 + ii of row b at base[(b * P + ii) * C]
-        double row[n];
-#pragma unroll
-        for (int a = 0; a < n; ++a) row[a] = INc[Cfg::ofs(j, a)];
-        double ip[NA], own[NA];
-#pragma unroll
-        for (int ii = 0; ii < NA - 1; ++ii) {
-            double sy = 0.0;
-#pragma unroll
-            for (int b = 0; b < n; ++b) sy = fma(sc.KY[j][b], base[(b * P + ii) * C], sy);
-            ip[ii] = wxv[ii] * sy;
-            own[ii] = base[(j * P + ii) * C];
-        }
-        {
-            constexpr int ii = NA - 1;
-            double sy = 0.0;
-            if (isface) {                                        // warp-uniform
-#pragma unroll
-                for (int b = 0; b < n; ++b) sy = fma(sc.KY[j][b], INc[(n * P + b) * C], sy);
-                own[ii] = INc[(n * P + j) * C];
-            } else {
-#pragma unroll
-                for (int b = 0; b < n; ++b) sy = fma(sc.KY[j][b], base[(b * P + ii) * C], sy);
-                own[ii] = base[(j * P + ii) * C];
-            }
-            ip[ii] = wxv[ii] * sy;
-        }
-        // x-contraction: row a0 + ii of K_x, fetched with a register index
-#pragma unroll
-        for (int ii = 0; ii < NA; ++ii) {
-            double sx = 0.0;
-#pragma unroll
-            for (int a = 0; a < n; ++a) sx = fma(sc.KX[a0 + ii][a], row[a], sx);
-            ip[ii] = fma(wyj, sx, ip[ii]);
-        }
-        double zr[NA];
-#pragma unroll
-        for (int ii = 0; ii < NA; ++ii) zr[ii] = wxy[ii] * own[ii];
-        if (lower) {
-#pragma unroll
-            for (int k = 0; k < n; ++k)
-#pragma unroll
-                for (int ii = 0; ii < NA; ++ii) acc[k][ii] = fma(sc.KZ[k][P], zr[ii], acc[k][ii]);
-#pragma unroll
-            for (int ii = 0; ii < NA; ++ii) acc[P][ii] = fma(sc.WZ[P], ip[ii], acc[P][ii]);
-            emit(ar, g0 + t - P, P);
-#pragma unroll
-            for (int ii = 0; ii < NA; ++ii) acc[0][ii] = acc[P][ii];
-#pragma unroll
-            for (int k = 1; k < n; ++k)
-#pragma unroll
-                for (int ii = 0; ii < NA; ++ii) acc[k][ii] = 0.0;
-        }
-        if (upper) {
-#pragma unroll
-            for (int k = 0; k < n; ++k) {
-                const double kz = sc.KZ[k][c];
-#pragma unroll
-                for (int ii = 0; ii < NA; ++ii) acc[k][ii] = fma(kz, zr[ii], acc[k][ii]);
-            }
-            const double wzc = sc.WZ[c];
-#pragma unroll
-            for (int ii = 0; ii < NA; ++ii) ip[ii] *= wzc;
-            if (jown) {
-                const double pz = sc.PZ[c] * pyj, fz = sc.FZ[c] * fyj * cin;
-#pragma unroll
-                for (int ii = 0; ii < NA; ++ii) {
-                    if (!(isface && ii == NA - 1)) {              // the face column is not owned
-                        const double* e = base + (j * P + ii) * C;
-                        const double in_own = own[ii];
-                        const double o_same = e[(col ^ (C / 2)) - col];
-                        const double o_flip = e[(col ^ (C / 2 + 1)) - col];
-                        const double* fn = Fs + (j * P + a0 + ii) * 4;
-                        const double diag = fn[s_spin];
-                        const double2 bxy = *reinterpret_cast<const double2*>(fn + 2);
-                        const double pot = fma(diag, in_own, fma(bxy.x, o_same, (sg * bxy.y) * o_flip));
-                        double val = fma(pz * sc.PX[a0 + ii], pot, ip[ii]);
-                        val = fma(fz * sc.FX[a0 + ii], in_own, val);
-                        if (ar.useR) val = fma(cR, Rs[(j * P + a0 + ii) * C + col], val);
-                        ip[ii] = val;
-                    }
-                }
-            }
-#pragma unroll
-            for (int k = 0; k < P; ++k) {
-                if (c == k) {
-#pragma unroll
-                    for (int ii = 0; ii < NA; ++ii) acc[k][ii] += ip[ii];
-                }
-            }
-        }
-        __syncwarp();
-        if ((threadIdx.x & 31) == 0) mbar_arrive(&empty_bar[s]);
-    }
-
-    __device__ __forceinline__ void run(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, uint64_t* full_bar,
-                                        uint64_t* empty_bar, int T) {
-        int c = 0;
-#pragma unroll 1
-        for (int t = 0; t < T; ++t) {
-            plane(sc, ar, smem, full_bar, empty_bar, t, c, c == 0 && t > 0, t < T - 1);
-            c = (c + 1 == P) ? 0 : c + 1;
-        }
-        emit(ar, g0 + T - 1, 1);
-    }
-};
-
-// ---------------------------------------------------------------------------------------------
 // FP32 product (CHFSI_FP32): the Laplacian of fl32(in) is computed and accumulated in FP32 from
 // the converter warp's FP32 copy of the plane; the pointwise potential, the in-term and the R-term of eq. 11 are
 // computed in FP64 from the FP64 stage and parked in the thread's own slots of PW until the cell is emitted, where
@@ -891,11 +674,6 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
     const int row = (warp % Cfg::WPH) * Cfg::RPW + lane / C;
     const int col = lane % C;
     (void)h; (void)row;
-    if constexpr (!F32 && XSPLIT > 1 && (n % XSPLIT) == 0) {
-        MarchConsumerU<P, CC, XSPLIT, HASPH> cs;
-        cs.init(sc, ar, h, row, col, ex, ey, chunk, g0, xwrap, ywrap);
-        cs.run(sc, ar, smem, full_bar, empty_bar, T);
-    } else {
 #define MARCH_PART(HH)                                                                                              \
     if (HH < XSPLIT && h == HH) {                                                                                   \
         if (F32)                                                                                                    \
@@ -908,7 +686,6 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
     }
     MARCH_PART(0) MARCH_PART(1) MARCH_PART(2)
 #undef MARCH_PART
-    }
 }
 
 // ---------------------------------------------------------------------------------------------
