@@ -285,3 +285,50 @@ def test_config1_full_size_sampled_columns(env):
     oracle on 3 sampled columns."""
     _, _, B = env
     _sampled_config_case(env, inp.CONFIGS[1], [0, 77, 127], [(B.FP64, TOL64), (B.FP32, TOL32)], 128)
+
+
+# ------------------------------------------------------------------------------- error behaviour (include/chfsi.h)
+def test_error_codes_on_device_calls(env):
+    """Every call returns a status and leaves the outputs alone on error: ESTATE before ham_set, EINVAL for bad
+    degree / bounds / leading dimension / chunk / workspace / missing Lambda, EUNSUPPORTED for the TF32 modes."""
+    torch, fo, B = env
+    cfg = inp.tiny_config(ncell=2, p=4, L=4.0, nvec=8, natoms=1, nproj=4)
+    mesh = B.chfsi_mesh_create(cfg.ncell, cfg.L, cfg.p, cfg.kfrac, 0)
+    try:
+        X = torch.from_numpy(inp.make_vectors(cfg.nnodes, 8)).cuda()
+        Y = torch.full_like(X, 3.0)
+        work = torch.empty(1 << 24, dtype=torch.uint8, device="cuda")
+
+        def status(fn, *a, **k):
+            try:
+                fn(*a, **k)
+                return B.OK
+            except B.ChfsiError as e:
+                return e.status
+
+        assert status(B.chfsi_apply_H, mesh, B.FP64, X, Y, work) == B.ESTATE
+        xyz = B.chfsi_mesh_node_coords(mesh)
+        hi = inp.make_hamiltonian(cfg, xyz)
+        B.chfsi_ham_set(mesh, hi.V, hi.Bx, hi.By, hi.Bz, hi.supp_off, hi.supp_node, hi.nproj, hi.P, hi.D)
+        lam = np.zeros(8)
+        filt = lambda **kw: status(B.chfsi_cheb_filter, mesh, kw.get("prec", B.FP64), kw.get("recur", B.RECUR_RESIDUAL),
+                                   kw.get("degree", 4), kw.get("a", 1.0), kw.get("b", 50.0), kw.get("a0", -2.0), X,
+                                   kw.get("lam", lam), Y, kw.get("work", work), chunk=kw.get("chunk", 0),
+                                   ldx=kw.get("ldx"), nvec=kw.get("nvec"))
+        assert filt() == B.OK
+        Y.fill_(3.0)
+        assert filt(degree=0) == B.EINVAL
+        assert filt(a=50.0, b=1.0) == B.EINVAL                       # b <= a
+        assert filt(a0=2.0) == B.EINVAL                              # a0 >= a
+        assert filt(ldx=4) == B.EINVAL                               # ld < nvec
+        assert filt(chunk=3) == B.EINVAL                             # chunk < nvec must be a multiple of 4
+        assert filt(lam=None) == B.EINVAL                            # eq. 11 needs Lambda
+        assert filt(work=work[:1024]) == B.EINVAL                    # workspace too small
+        assert filt(work=work[8:]) == B.EINVAL                       # workspace not 256-byte aligned
+        assert filt(prec=B.TF32) == B.EUNSUPPORTED and filt(prec=B.TF32X3) == B.EUNSUPPORTED
+        assert status(B.chfsi_apply_H, mesh, B.FP64, X, X, work) == B.EINVAL      # apply_H cannot alias
+        torch.cuda.synchronize()
+        assert bool((Y == 3.0).all())                                # failed calls wrote nothing
+        assert filt(recur=B.RECUR_STANDARD, lam=None) == B.OK        # eq. 10 takes no Lambda
+    finally:
+        B.chfsi_mesh_destroy(mesh)
