@@ -132,7 +132,7 @@ struct MarchCfg {
 };
 
 // Per-thread state of a consumer (part H of row j, lane = batch column).
-template <int P, int CC, int XSPLIT, bool HASPH, int H>
+template <int P, int CC, int XSPLIT, bool HASPH, int H, bool FULLV>
 struct MarchConsumer {
     using Cfg = MarchCfg<P, CC, XSPLIT>;
     static constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES;
@@ -210,7 +210,13 @@ struct MarchConsumer {
                         const bool fc = A0 + ii == P;
                         val = fma(other, fc ? bi_ : ai_, val * (fc ? br_ : ar_));
                     }
-                    if (vok) atomicAdd(dst, val);
+                    if (FULLV) {
+                        // every vector of the chunk exists (nvec % NV == 0): no predicate, so no branch around the RED
+                        // (padding rows of a C = 16 warp add an exact zero)
+                        atomicAdd(dst, (Cfg::RPW == 1 || valid) ? val : 0.0);
+                    } else if (vok) {
+                        atomicAdd(dst, val);
+                    }
                 }
             }
         }
@@ -348,7 +354,7 @@ struct MarchConsumer {
 // the converter warp's FP32 copy of the plane; the pointwise potential, the in-term and the R-term of eq. 11 are
 // computed in FP64 from the FP64 stage and parked in the thread's own slots of PW until the cell is emitted, where
 // the FP32 Laplacian is widened exactly, scaled by cH in FP64 and both are sent out with one RED.ADD.F64.
-template <int P, int CC, int XSPLIT, bool HASPH, int H>
+template <int P, int CC, int XSPLIT, bool HASPH, int H, bool FULLV>
 struct MarchConsumerF32 {
     using Cfg = MarchCfg<P, CC, XSPLIT>;
     static constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES32, NFB = Cfg::NFB;
@@ -436,7 +442,13 @@ struct MarchConsumerF32 {
                         const bool fc = A0 + ii == P;
                         val = fma(other, fc ? bi_ : ai_, val * (fc ? br_ : ar_));
                     }
-                    if (vok) atomicAdd(dst, val);
+                    if (FULLV) {
+                        // every vector of the chunk exists (nvec % NV == 0): no predicate, so no branch around the RED
+                        // (padding rows of a C = 16 warp add an exact zero)
+                        atomicAdd(dst, (Cfg::RPW == 1 || valid) ? val : 0.0);
+                    } else if (vok) {
+                        atomicAdd(dst, val);
+                    }
                 }
             }
         }
@@ -579,25 +591,25 @@ __device__ __forceinline__ void march_convert(const MarchArgs& ar, unsigned char
     }
 }
 
-template <int P, int CC, int XSPLIT, bool HASPH, int H>
+template <int P, int CC, int XSPLIT, bool HASPH, int H, bool FULLV>
 __device__ __forceinline__ void march_consume(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, uint64_t* full_bar,
                                            uint64_t* empty_bar, int row, int col, int ex, int ey, int chunk, int g0, int T,
                                            bool xwrap, bool ywrap) {
-    MarchConsumer<P, CC, XSPLIT, HASPH, H> cs;
+    MarchConsumer<P, CC, XSPLIT, HASPH, H, FULLV> cs;
     cs.init(sc, ar, row, col, ex, ey, chunk, g0, xwrap, ywrap);
     cs.run(sc, ar, smem, full_bar, empty_bar, T);
 }
 
-template <int P, int CC, int XSPLIT, bool HASPH, int H>
+template <int P, int CC, int XSPLIT, bool HASPH, int H, bool FULLV>
 __device__ __forceinline__ void march_consume32(const StepConst& sc, const MarchArgs& ar, unsigned char* smem, float* FB, double* PW,
                                                 uint64_t* full_bar, uint64_t* empty_bar, uint64_t* cfull_bar, uint64_t* cempty_bar,
                                                 int row, int col, int ex, int ey, int chunk, int g0, int T, bool xwrap, bool ywrap) {
-    MarchConsumerF32<P, CC, XSPLIT, HASPH, H> cs;
+    MarchConsumerF32<P, CC, XSPLIT, HASPH, H, FULLV> cs;
     cs.init(sc, ar, PW, row, col, ex, ey, chunk, g0, xwrap, ywrap);
     cs.run(sc, ar, smem, FB, full_bar, empty_bar, cfull_bar, cempty_bar, T);
 }
 
-template <int P, int CC, int XSPLIT, bool HASPH, bool F32>
+template <int P, int CC, int XSPLIT, bool HASPH, bool F32, bool FULLV>
 __global__ void __launch_bounds__(F32 ? MarchCfg<P, CC, XSPLIT>::THREADS32 : MarchCfg<P, CC, XSPLIT>::THREADS, 1)
 cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ MarchArgs ar,
                   const __grid_constant__ MarchMaps mp) {
@@ -677,11 +689,11 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
 #define MARCH_PART(HH)                                                                                              \
     if (HH < XSPLIT && h == HH) {                                                                                   \
         if (F32)                                                                                                    \
-            march_consume32<P, CC, XSPLIT, HASPH, (HH < XSPLIT ? HH : 0)>(sc, ar, smem, FB, PW, full_bar, empty_bar, \
+            march_consume32<P, CC, XSPLIT, HASPH, (HH < XSPLIT ? HH : 0), FULLV>(sc, ar, smem, FB, PW, full_bar, empty_bar, \
                                                                           cfull_bar, cempty_bar, row, col, ex, ey,  \
                                                                           chunk, g0, T, xwrap, ywrap);              \
         else                                                                                                        \
-            march_consume<P, CC, XSPLIT, HASPH, (HH < XSPLIT ? HH : 0)>(sc, ar, smem, full_bar, empty_bar, row, col, ex, ey, \
+            march_consume<P, CC, XSPLIT, HASPH, (HH < XSPLIT ? HH : 0), FULLV>(sc, ar, smem, full_bar, empty_bar, row, col, ex, ey, \
                                                                         chunk, g0, T, xwrap, ywrap);               \
     }
     MARCH_PART(0) MARCH_PART(1) MARCH_PART(2)
@@ -805,8 +817,10 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
     const size_t smem = F32 ? (size_t)Cfg::STAGES32 * Cfg::STAGE_BYTES + Cfg::NFB * Cfg::FB_BYTES + Cfg::PW_BYTES
                             : (size_t)Cfg::STAGES * Cfg::STAGE_BYTES;
     static bool attr_done[128] = {false};   // per template instantiation
-    auto kern = m->mc.has_phase ? cell_march_kernel<P, CC, XSPLIT, true, F32> : cell_march_kernel<P, CC, XSPLIT, false, F32>;
-    const int slot = (m->device & 63) * 2 + (m->mc.has_phase ? 1 : 0);
+    const bool full = (a.nvec % Cfg::NV) == 0;          // every CTA's vector tile is complete: unpredicated REDs
+    auto kern = m->mc.has_phase ? (full ? cell_march_kernel<P, CC, XSPLIT, true, F32, true> : cell_march_kernel<P, CC, XSPLIT, true, F32, false>)
+                                : (full ? cell_march_kernel<P, CC, XSPLIT, false, F32, true> : cell_march_kernel<P, CC, XSPLIT, false, F32, false>);
+    const int slot = (m->device & 31) * 4 + (m->mc.has_phase ? 2 : 0) + (full ? 1 : 0);
     if (!attr_done[slot]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
