@@ -180,7 +180,7 @@ struct MarchConsumer {
     // The REDs are left individually predicated on purpose: ptxas then spreads them between the FMAs of the
     // surrounding z-push; hoisting the predicate into one branch bunches 6(p+1) REDs together and costs 15 %.
     __device__ __forceinline__ void emit(const MarchArgs& ar, int gzbase, int nk) {
-        const long long xstride = 4 * ar.ld_out;                       // doubles between consecutive nodes
+        const long long xsb = 32 * ar.ld_out;                          // bytes between consecutive nodes
         const long long x0 = (long long)ex * P + A0;
 #pragma unroll
         for (int k = 0; k < n; ++k) {
@@ -197,12 +197,14 @@ struct MarchConsumer {
                     if (ri) { ai_ = -ai_; bi_ = -bi_; }
                 }
                 (void)ar_; (void)ai_; (void)br_; (void)bi_; (void)anyw;
-                double* line = outcol + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xstride;
-                double* pnode = line + x0 * xstride;
+                // running byte pointer along the x-line: two integer adds per RED instead of a full index computation
+                char* line = reinterpret_cast<char*>(outcol) + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xsb;
+                char* pnode = line + x0 * xsb;
 #pragma unroll
                 for (int ii = 0; ii < NAH; ++ii) {
                     const bool wx = (A0 + ii == P) && xwrap;
-                    double* dst = wx ? line : pnode + ii * xstride;
+                    double* dst = reinterpret_cast<double*>(wx ? line : pnode);
+                    pnode += xsb;
                     double val = acc[k][ii];
                     if (HASPH && anyw) {
                         // times conj(phase), branch-free: (pr, pi) is (1, 0) where nothing wrapped
@@ -409,7 +411,7 @@ struct MarchConsumerF32 {
 
     // emit planes [0, nk): out += cH * (double)acc + PW (owned nodes only; with_pw false for the segment's top face)
     __device__ __forceinline__ void emit(const StepConst& sc, const MarchArgs& ar, int gzbase, int nk, bool with_pw) {
-        const long long xstride = 4 * ar.ld_out;
+        const long long xsb = 32 * ar.ld_out;                          // bytes between consecutive nodes
         const long long x0 = (long long)ex * P + A0;
 #pragma unroll
         for (int k = 0; k < n; ++k) {
@@ -426,12 +428,14 @@ struct MarchConsumerF32 {
                     if (ri) { ai_ = -ai_; bi_ = -bi_; }
                 }
                 (void)ar_; (void)ai_; (void)br_; (void)bi_; (void)anyw;
-                double* line = outcol + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xstride;
-                double* pnode = line + x0 * xstride;
+                // running byte pointer along the x-line: two integer adds per RED instead of a full index computation
+                char* line = reinterpret_cast<char*>(outcol) + ((long long)gz * ar.n1[1] + gy) * ar.n1[0] * xsb;
+                char* pnode = line + x0 * xsb;
 #pragma unroll
                 for (int ii = 0; ii < NAH; ++ii) {
                     const bool wx = (A0 + ii == P) && xwrap;
-                    double* dst = wx ? line : pnode + ii * xstride;
+                    double* dst = reinterpret_cast<double*>(wx ? line : pnode);
+                    pnode += xsb;
                     double val = sc.cH * (double)acc[k][ii];
                     if (A0 + ii < P && k < P) {
                         if (with_pw && jown) val += pw[(k * P * P + A0 + ii) * C];
