@@ -223,6 +223,9 @@ chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
     {
         DeviceGuard g(m->device);
         for (cudaEvent_t e : m->prof_ev) cudaEventDestroy(e);
+        if (m->ev_proj) cudaEventDestroy(m->ev_proj);
+        if (m->ev_back) cudaEventDestroy(m->ev_back);
+        if (m->side) cudaStreamDestroy(m->side);
         cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF);
         free_nonlocal(m->nl);
     }
@@ -356,6 +359,13 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
         CU(upload(&nl.P32, P32));
         CU(upload(&nl.D64, D64));
     }
+    if (!m->side) {   // side stream of the projector back-pass (setup call: allocation is allowed here)
+        int lo = 0, hi = 0;
+        CU(cudaDeviceGetStreamPriorityRange(&lo, &hi));              // lo = lowest priority (largest number)
+        CU(cudaStreamCreateWithPriority(&m->side, cudaStreamNonBlocking, lo));
+        CU(cudaEventCreateWithFlags(&m->ev_proj, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&m->ev_back, cudaEventDisableTiming));
+    }
     CU(cudaDeviceSynchronize());
     m->ham_set = true;
     return CHFSI_OK;
@@ -374,18 +384,32 @@ chfsi_status chfsi_workspace_bytes(const chfsi_mesh* m, chfsi_prec prec, chfsi_r
 // cell kernel, projector back pass.  `out` must already hold the value being accumulated into.
 static chfsi_status accumulate_H(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& ca, double* Cbuf, cudaStream_t st) {
     const bool nlocal = m->nl.nitems > 0;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    cudaStreamIsCapturing(st, &cap);
+    const bool fork = nlocal && m->side != nullptr && !m->prof_on && cap == cudaStreamCaptureStatusNone;
     if (nlocal) {
         CU(cudaMemsetAsync(Cbuf, 0, (size_t)m->nl.crows * ca.nvec * 16, st));
         count_launch();
         ProjArgs pa{ca.in, ca.ld_in, Cbuf, ca.nvec, (ca.flags & kScaleIn) ? 0 : 1};
         CU(launch_proj(m, prec, pa, st));
     }
+    if (fork) {
+        CU(cudaEventRecord(m->ev_proj, st));
+    }
     CU(launch_cell(m, prec, ca, st));
     if (nlocal) {
         double* Gbuf = reinterpret_cast<double*>(reinterpret_cast<char*>(Cbuf) +
                                                  align256((size_t)m->nl.crows * ca.nvec * 16));
         BackArgs ba{Cbuf, Gbuf, ca.out, ca.ld_out, ca.cH, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
-        CU(launch_back(m, prec, ba, st));
+        if (fork) {
+            // both kernels only accumulate into `out` (RED), so their order does not matter
+            CU(cudaStreamWaitEvent(m->side, m->ev_proj, 0));
+            CU(launch_back(m, prec, ba, m->side));
+            CU(cudaEventRecord(m->ev_back, m->side));
+            CU(cudaStreamWaitEvent(st, m->ev_back, 0));
+        } else {
+            CU(launch_back(m, prec, ba, st));
+        }
     }
     return CHFSI_OK;
 }
