@@ -387,30 +387,32 @@ static chfsi_status accumulate_H(const chfsi_mesh* m, chfsi_prec prec, const Cel
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     cudaStreamIsCapturing(st, &cap);
     const bool fork = nlocal && m->side != nullptr && !m->prof_on && cap == cudaStreamCaptureStatusNone;
+    double* Gbuf = reinterpret_cast<double*>(reinterpret_cast<char*>(Cbuf) +
+                                             align256((size_t)m->nl.crows * ca.nvec * 16));
+    ProjArgs pa{ca.in, ca.ld_in, Cbuf, ca.nvec, (ca.flags & kScaleIn) ? 0 : 1};
+    BackArgs ba{Cbuf, Gbuf, ca.out, ca.ld_out, ca.cH, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
+    if (fork) {
+        // The nonlocal term (zero C, project, back-project) depends on `in` only and, like the cell kernel, only
+        // accumulates into `out` (RED): it runs on the mesh's low-priority stream beside the cell kernel and takes
+        // the SMs that kernel's last wave leaves idle.
+        CU(cudaEventRecord(m->ev_proj, st));
+        CU(launch_cell(m, prec, ca, st));                            // first, so that its CTAs take the SMs
+        CU(cudaStreamWaitEvent(m->side, m->ev_proj, 0));
+        CU(cudaMemsetAsync(Cbuf, 0, (size_t)m->nl.crows * ca.nvec * 16, m->side));
+        count_launch();
+        CU(launch_proj(m, prec, pa, m->side));
+        CU(launch_back(m, prec, ba, m->side));
+        CU(cudaEventRecord(m->ev_back, m->side));
+        CU(cudaStreamWaitEvent(st, m->ev_back, 0));
+        return CHFSI_OK;
+    }
     if (nlocal) {
         CU(cudaMemsetAsync(Cbuf, 0, (size_t)m->nl.crows * ca.nvec * 16, st));
         count_launch();
-        ProjArgs pa{ca.in, ca.ld_in, Cbuf, ca.nvec, (ca.flags & kScaleIn) ? 0 : 1};
         CU(launch_proj(m, prec, pa, st));
     }
-    if (fork) {
-        CU(cudaEventRecord(m->ev_proj, st));
-    }
     CU(launch_cell(m, prec, ca, st));
-    if (nlocal) {
-        double* Gbuf = reinterpret_cast<double*>(reinterpret_cast<char*>(Cbuf) +
-                                                 align256((size_t)m->nl.crows * ca.nvec * 16));
-        BackArgs ba{Cbuf, Gbuf, ca.out, ca.ld_out, ca.cH, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
-        if (fork) {
-            // both kernels only accumulate into `out` (RED), so their order does not matter
-            CU(cudaStreamWaitEvent(m->side, m->ev_proj, 0));
-            CU(launch_back(m, prec, ba, m->side));
-            CU(cudaEventRecord(m->ev_back, m->side));
-            CU(cudaStreamWaitEvent(st, m->ev_back, 0));
-        } else {
-            CU(launch_back(m, prec, ba, st));
-        }
-    }
+    if (nlocal) CU(launch_back(m, prec, ba, st));
     return CHFSI_OK;
 }
 
