@@ -21,7 +21,7 @@
  *     x = (e + (xi_a + 1)/2) * h  for cell e and GLL node xi_a, a = 0..p-1.
  *   - chfsi_apply_H and chfsi_cheb_filter allocate nothing, never synchronise the host with the
  *     device, and enqueue all work on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
- *     legacy default stream) -- except that the projector back-pass of a step may run on a
+ *     legacy default stream) -- except that the nonlocal term of a step may run on a
  *     low-priority stream owned by the mesh, forked from and joined back into `cuda_stream` inside
  *     the call, so that work queued on `cuda_stream` after the call still sees it complete.  Setup
  *     calls (mesh_create, ham_set, destroy) may allocate and synchronise.

@@ -116,8 +116,8 @@ struct chfsi_mesh {
     mutable bool prof_on = false;
     mutable std::vector<cudaEvent_t> prof_ev;      // start/stop pairs
     mutable double prof_bytes = 0.0;
-    // low-priority side stream: the projector back-pass of a step only needs the coefficients, so it runs beside the
-    // cell kernel and fills the SMs that kernel's last wave leaves idle
+    // low-priority side stream: the nonlocal term of a step runs beside the cell kernel and fills the SMs that
+    // kernel's last wave leaves idle (created in chfsi_ham_set)
     mutable cudaStream_t side = nullptr;
     mutable cudaEvent_t ev_proj = nullptr, ev_back = nullptr;
 };
