@@ -627,11 +627,15 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // blockIdx -> (ex fastest, ey, seg, chunk): neighbours in x/y run together, so shared faces hit in L2
+    // With C = 16 a 128-byte line holds the rows of TWO chunks: the pair runs side by side (pair index fastest).
     int bid = blockIdx.x;
+    int cpair = 0;
+    if (C == 16) { cpair = bid & 1; bid >>= 1; }
     const int ex = bid % ar.nc[0]; bid /= ar.nc[0];
     const int ey = bid % ar.nc[1]; bid /= ar.nc[1];
     const int seg = bid % ar.nseg;
-    const int chunk = bid / ar.nseg;
+    const int chunk = C == 16 ? 2 * (bid / ar.nseg) + cpair : bid / ar.nseg;
+    if (chunk >= ar.nchunks) return;              // odd chunk count: the last pair is half empty
     const int T = ar.cps * P + 1;                 // planes this CTA marches through
     const int g0 = seg * ar.cps * P;              // first global plane
     const bool xwrap = ex == ar.nc[0] - 1, ywrap = ey == ar.nc[1] - 1;
@@ -734,7 +738,7 @@ static bool make_map3(CUtensorMap* map, const chfsi_mesh* m, const double* base,
     cuuint32_t estr[3] = {1u, 1u, 1u};
     return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), gdim, gstr, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-               box_cols * 8 >= 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -830,7 +834,7 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
         if (e != cudaSuccess) return e;
         attr_done[slot] = true;
     }
-    const long long grid = base * nseg;
+    const long long grid = CC == 16 ? (long long)ar.nc[0] * ar.nc[1] * nseg * 2 * ((ar.nchunks + 1) / 2) : base * nseg;
     kern<<<(unsigned)grid, F32 ? Cfg::THREADS32 : Cfg::THREADS, smem, st>>>(sc, ar, mp);
     return cudaGetLastError();
 }
