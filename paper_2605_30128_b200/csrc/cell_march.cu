@@ -43,6 +43,7 @@ struct StepConst {
 struct MarchArgs {
     int nc[3], n1[3];
     int has_phase;
+    int phd[3];                 // direction d has a nontrivial Bloch phase (phi_d != 1)
     double ph_re[3], ph_im[3];
     int nseg, cps;              // z segments, cells per segment
     int nvec, nchunks;
@@ -143,12 +144,13 @@ struct MarchConsumer {
     double pAr, pAi, pBr, pBi;   // Bloch phase of this row's plain and x-face entries (HASPH)
     double* outcol;
     int j, col, s_spin, ri, ex, gy, g0;
-    bool vok, jown, wy, xwrap, ywrap, valid;
+    bool vok, jown, wy, xwrap, ywrap, valid, xph, yph;
 
     __device__ __forceinline__ void init(const StepConst& sc, const MarchArgs& ar, int row, int col_, int ex_, int ey,
                                          int chunk, int g0_, bool xw, bool yw) {
         valid = row < n;
         j = valid ? row : n - 1; col = col_; ex = ex_; g0 = g0_; xwrap = xw; ywrap = yw;
+        xph = xw && ar.phd[0]; yph = yw && ar.phd[1];   // wraps that actually carry a phase
         s_spin = col / (C / 2); ri = col & 1;
         sg = ((ri == 0) != (s_spin == 0)) ? -1.0 : 1.0;
         const int vl = (col % (C / 2)) >> 1;
@@ -186,7 +188,7 @@ struct MarchConsumer {
         for (int k = 0; k < n; ++k) {
             if (k < nk) {
                 int gz = gzbase + k; const bool wz = gz == ar.n1[2]; if (wz) gz = 0;
-                const bool anyw = xwrap | ywrap | wz;                  // CTA-uniform: interior CTAs skip the phase arithmetic
+                const bool anyw = xph | yph | (wz && ar.phd[2]);                  // CTA-uniform: interior CTAs skip the phase arithmetic
                 double ar_ = pAr, ai_ = pAi, br_ = pBr, bi_ = pBi;      // conj-phase of plain / x-face columns of this row
                 if (HASPH) {
                     if (wz) {
@@ -237,12 +239,12 @@ struct MarchConsumer {
         if (HASPH) {
             // Bloch phase on wrapped entries (x: column a = P; y: row j = P; z: the wrapped plane), fixed up in place;
             // each part fixes its own x-positions of its row
-            const bool wz = (g0 + t) == ar.n1[2];
-            if (xwrap | ywrap | wz) {                                    // CTA-uniform
-                const bool wyy = ywrap && j == P;
+            const bool wz = ar.phd[2] && (g0 + t) == ar.n1[2];
+            if (xph | yph | wz) {                                        // CTA-uniform
+                const bool wyy = yph && j == P;
 #pragma unroll
                 for (int ii = 0; ii < NAH; ++ii) {
-                    const bool wx = xwrap && (A0 + ii == P);
+                    const bool wx = xph && (A0 + ii == P);
                     const double val = IN[Cfg::ofs(j, A0 + ii) + col];
                     const double other = __shfl_xor_sync(0xffffffffu, val, 1);
                     if ((wx | wyy | wz) && valid) {
@@ -370,12 +372,13 @@ struct MarchConsumerF32 {
     double* outcol;
     double* pw;                  // PW + (j * P) * C + col : this thread's pointwise slots, [c][.][a][.]
     int j, col, s_spin, ri, ex, gy, g0;
-    bool vok, jown, wy, xwrap, ywrap, valid;
+    bool vok, jown, wy, xwrap, ywrap, valid, xph, yph;
 
     __device__ __forceinline__ void init(const StepConst& sc, const MarchArgs& ar, double* PW, int row, int col_, int ex_, int ey,
                                          int chunk, int g0_, bool xw, bool yw) {
         valid = row < n;
         j = valid ? row : n - 1; col = col_; ex = ex_; g0 = g0_; xwrap = xw; ywrap = yw;
+        xph = xw && ar.phd[0]; yph = yw && ar.phd[1];   // wraps that actually carry a phase
         s_spin = col / (C / 2); ri = col & 1;
         sg = ((ri == 0) != (s_spin == 0)) ? -1.0 : 1.0;
         const int vl = (col % (C / 2)) >> 1;
@@ -417,7 +420,7 @@ struct MarchConsumerF32 {
         for (int k = 0; k < n; ++k) {
             if (k < nk) {
                 int gz = gzbase + k; const bool wz = gz == ar.n1[2]; if (wz) gz = 0;
-                const bool anyw = xwrap | ywrap | wz;                  // CTA-uniform: interior CTAs skip the phase arithmetic
+                const bool anyw = xph | yph | (wz && ar.phd[2]);                  // CTA-uniform: interior CTAs skip the phase arithmetic
                 double ar_ = pAr, ai_ = pAi, br_ = pBr, bi_ = pBi;      // conj-phase of plain / x-face columns of this row
                 if (HASPH) {
                     if (wz) {
@@ -571,7 +574,7 @@ __device__ __forceinline__ void march_convert(const MarchArgs& ar, unsigned char
         mbar_wait(&full_bar[s], (t / STAGES) & 1);
         const double2* IN2 = reinterpret_cast<const double2*>(smem + (size_t)s * Cfg::STAGE_BYTES);
         float2* FB2 = reinterpret_cast<float2*>(FBbase + (size_t)f * (Cfg::FB_BYTES / 4));
-        const bool wz = HASPH && (g0 + t) == ar.n1[2];
+        const bool wz = HASPH && ar.phd[2] && (g0 + t) == ar.n1[2];
 #pragma unroll 4
         for (int e = cw * 32 + lane; e < n * n * HC; e += 32 * Cfg::NCW) {
             double2 v = IN2[e];
@@ -685,7 +688,7 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
 
     if (F32 && warp > Cfg::CWARPS) {
         march_convert<P, CC, XSPLIT, HASPH>(ar, smem, FB, full_bar, cfull_bar, cempty_bar, warp - Cfg::CWARPS - 1, lane, g0, T,
-                                            xwrap, ywrap);
+                                            xwrap && ar.phd[0], ywrap && ar.phd[1]);
         return;
     }
 
@@ -805,6 +808,7 @@ static cudaError_t launch_march_t(const chfsi_mesh* m, const CellArgs& a, cudaSt
         ar.ph_re[d] = m->mc.ph_re[d]; ar.ph_im[d] = m->mc.ph_im[d];
     }
     ar.has_phase = m->mc.has_phase;
+    for (int d = 0; d < 3; ++d) ar.phd[d] = (m->mc.ph_re[d] != 1.0 || m->mc.ph_im[d] != 0.0) ? 1 : 0;
     ar.nvec = a.nvec; ar.nchunks = (a.nvec + Cfg::NV - 1) / Cfg::NV;
     ar.useR = (a.R != nullptr && a.cR != nullptr) ? 1 : 0;
     ar.fields = m->dF; ar.cin = a.cin; ar.cR = a.cR; ar.out = a.out; ar.ld_out = a.ld_out;
