@@ -332,3 +332,26 @@ def test_error_codes_on_device_calls(env):
         assert filt(recur=B.RECUR_STANDARD, lam=None) == B.OK        # eq. 10 takes no Lambda
     finally:
         B.chfsi_mesh_destroy(mesh)
+
+
+@pytest.mark.parametrize("p,ncell,nvec", [(2, (8, 8, 4), 40), (4, (10, 6, 6), 48), (6, (8, 8, 4), 40)])
+def test_z_segments_of_more_than_one_cell(env, p, ncell, nvec):
+    """Grids where the march kernel splits the z-range into segments of 2 or 3 cells (between the one-cell segments
+    of the small meshes and the whole-column marches of the BASELINE configs): the segment's top-face partial sums
+    and the carry of the top plane across cells are both exercised."""
+    _, fo, B = env
+    cfg = inp.tiny_config(ncell=ncell, p=p, L=tuple(1.5 * c for c in ncell), kfrac=(0.0, 0.25, 0.5), nvec=nvec,
+                          natoms=2, nproj=8, ngauss=3)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, nvec)
+        ref = fo.apply_MinvH(pb.oham, X)
+        assert relerr(pb.gpu_apply(X, B.FP64), ref) < 1e-13
+        assert relerr(pb.gpu_apply(X, B.FP32), ref) < 2e-6
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref11 = fo.cheb_filter_residual(pb.oham, X, lam, 5, a, b, a0)
+        assert relerr(pb.gpu_filter(X, lam, 5, a, b, a0, B.FP64, B.RECUR_RESIDUAL), ref11) < TOL64
+        assert relerr(pb.gpu_filter(X, lam, 5, a, b, a0, B.FP32, B.RECUR_RESIDUAL), ref11) < TOL32
+    finally:
+        pb.close()
