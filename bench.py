@@ -155,12 +155,17 @@ def run_ours(args, cfg):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-    B.lib()
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    if rank == 0:
+        from paper_2605_30128_b200 import build as _build
+        _build.build()                       # no-op when libchfsi.so is up to date
+    if dist is not None:
+        dist.barrier()
+    B.lib()
     dev = f"cuda:{local}"
     prec = B.PREC[args.prec]
     recur = B.RECUR_RESIDUAL if args.recur == "residual" else B.RECUR_STANDARD
