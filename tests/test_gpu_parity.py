@@ -231,6 +231,14 @@ def test_single_vector_and_wide_leading_dimension_in_filter(env):
             Y = Yd.cpu().numpy()
             assert relerr(Y[:, :, 3:12], ref[:, :, 2:11]) < tol
             assert np.all(Y[:, :, :3] == 5.0) and np.all(Y[:, :, 12:] == 5.0)
+            # eight columns: complete vector tiles (the kernel variant with unpredicated REDs) inside wider blocks
+            Yd.fill_(5.0)
+            B.chfsi_cheb_filter(pb.gmesh, prec, B.RECUR_RESIDUAL, 6, a, b, a0, Xd[:, :, 4:12], lam[4:12], Yd[:, :, 1:9],
+                                pb.work(prec, B.RECUR_RESIDUAL, 8), nvec=8, ldx=13, ldy=16)
+            torch.cuda.synchronize()
+            Y = Yd.cpu().numpy()
+            assert relerr(Y[:, :, 1:9], ref[:, :, 4:12]) < tol
+            assert np.all(Y[:, :, :1] == 5.0) and np.all(Y[:, :, 9:] == 5.0)
     finally:
         pb.close()
 
