@@ -37,7 +37,8 @@ struct StepConst {
     // FP32 Laplacian is widened
     float KXf[kMaxN][kMaxN], KYf[kMaxN][kMaxN], KZf[kMaxN][kMaxN];
     float WXf[kMaxN], WYf[kMaxN], WZf[kMaxN];
-    double cH;
+    double cH;                 // FP32 product: step coefficient / in_scale, applied in FP64 to the widened Laplacian
+    double in_scale;           // FP32 product: power of two applied (in FP64) to `in` before the cast
 };
 
 struct MarchArgs {
@@ -564,7 +565,7 @@ struct MarchConsumerF32 {
 template <int P, int CC, int XSPLIT, bool HASPH>
 __device__ __forceinline__ void march_convert(const MarchArgs& ar, unsigned char* smem, float* FBbase, uint64_t* full_bar,
                                               uint64_t* cfull_bar, uint64_t* cempty_bar, int cw, int lane, int g0, int T,
-                                              bool xwrap, bool ywrap) {
+                                              bool xwrap, bool ywrap, double isc) {
     using Cfg = MarchCfg<P, CC, XSPLIT>;
     constexpr int n = Cfg::n, C = Cfg::C, STAGES = Cfg::STAGES32, NFB = Cfg::NFB, HC = C / 2;
 #pragma unroll 1
@@ -591,7 +592,7 @@ __device__ __forceinline__ void march_convert(const MarchArgs& ar, unsigned char
                     v = make_double2(v.x * pr - v.y * pi, v.x * pi + v.y * pr);
                 }
             }
-            FB2[e] = make_float2((float)v.x, (float)v.y);
+            FB2[e] = make_float2((float)(v.x * isc), (float)(v.y * isc));   // isc: exact power-of-two rescaling
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&cfull_bar[f]);
@@ -688,7 +689,7 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
 
     if (F32 && warp > Cfg::CWARPS) {
         march_convert<P, CC, XSPLIT, HASPH>(ar, smem, FB, full_bar, cfull_bar, cempty_bar, warp - Cfg::CWARPS - 1, lane, g0, T,
-                                            xwrap && ar.phd[0], ywrap && ar.phd[1]);
+                                            xwrap && ar.phd[0], ywrap && ar.phd[1], sc.in_scale);
         return;
     }
 
@@ -774,7 +775,9 @@ static void build_step_const(const chfsi_mesh* m, const CellArgs& a, StepConst& 
     const int n = mc.n;
     const bool sin_ = (a.flags & kScaleIn) != 0, sout_ = (a.flags & kSoutInvM) != 0, massin = (a.flags & kMassIn) != 0;
     std::memset(&sc, 0, sizeof(sc));
-    sc.cH = a.cH;
+    const double isc = a.in_scale > 0.0 ? a.in_scale : 1.0;        // used by the FP32 product only
+    sc.cH = a.cH / isc;
+    sc.in_scale = isc;
     for (int d = 0; d < 3; ++d) {
         double (*K)[kMaxN] = d == 0 ? sc.KX : d == 1 ? sc.KY : sc.KZ;
         double* W = d == 0 ? sc.WX : d == 1 ? sc.WY : sc.WZ;

@@ -389,8 +389,9 @@ static chfsi_status accumulate_H(const chfsi_mesh* m, chfsi_prec prec, const Cel
     const bool fork = nlocal && m->side != nullptr && !m->prof_on && cap == cudaStreamCaptureStatusNone;
     double* Gbuf = reinterpret_cast<double*>(reinterpret_cast<char*>(Cbuf) +
                                              align256((size_t)m->nl.crows * ca.nvec * 16));
-    ProjArgs pa{ca.in, ca.ld_in, Cbuf, ca.nvec, (ca.flags & kScaleIn) ? 0 : 1};
-    BackArgs ba{Cbuf, Gbuf, ca.out, ca.ld_out, ca.cH, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
+    const double isc = (prec == CHFSI_FP32 && ca.in_scale > 0.0) ? ca.in_scale : 1.0;
+    ProjArgs pa{ca.in, ca.ld_in, Cbuf, ca.nvec, (ca.flags & kScaleIn) ? 0 : 1, isc};
+    BackArgs ba{Cbuf, Gbuf, ca.out, ca.ld_out, ca.cH / isc, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
     if (fork) {
         // The nonlocal term (zero C, project, back-project) depends on `in` only and, like the cell kernel, only
         // accumulates into `out` (RED): it runs on the mesh's low-priority stream beside the cell kernel and takes
@@ -559,6 +560,7 @@ chfsi_status chfsi_cheb_filter(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur
                 cs.R = (k >= 2) ? R : nullptr; cs.ld_R = nb;
                 cs.cin = dCIN(k); cs.cR = (k >= 2) ? dCR(k) : nullptr;
                 cs.cH = cHs[k]; cs.nvec = nb; cs.flags = kScaleIn;
+                cs.in_scale = std::ldexp(1.0, std::ilogb(std::fabs(s[k])));     // in = Z_k / s_k
                 stt = accumulate_H(m, prec, cs, Cbuf, st);
                 if (stt != CHFSI_OK) return stt;
                 zin = zout; zcur = zout;
@@ -598,6 +600,7 @@ chfsi_status chfsi_cheb_filter(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur
                 cs.out = in_even ? O : E; cs.ld_out = in_even ? ldO : ldE;
                 cs.R = nullptr; cs.ld_R = 0; cs.cin = dCIN(k + 1); cs.cR = nullptr;
                 cs.cH = cHs[k]; cs.nvec = nb; cs.flags = kSoutInvM;
+                cs.in_scale = std::ldexp(1.0, std::ilogb(std::fabs(s[k])));     // in = Y_k / s_k
                 stt = accumulate_H(m, prec, cs, Cbuf, st);
                 if (stt != CHFSI_OK) return stt;
             }

@@ -51,6 +51,10 @@ struct CellArgs {
     double cH;
     int nvec;
     int flags;
+    // FP32 product only: `in` is multiplied by this power of two (exactly, in FP64) before the cast to FP32 and the
+    // FP32 result by its reciprocal after widening, so that the scaled iterates Z_k / s_k stay
+    // inside the FP32 range at any degree.  1.0 (or 0 = unset) elsewhere.
+    double in_scale;
 };
 
 struct ProjItem { int atom; int start; int count; };   // a slice of an atom's support list
@@ -82,6 +86,7 @@ struct ProjArgs {
     double* C;                          // [crows][nvec] complex128, zeroed by the driver
     int nvec;
     int mass_u;                         // 1: u = m_I * in (apply on X); 0: u = in (Z-form)
+    double in_scale;                    // see CellArgs::in_scale (the back pass gets cH / in_scale)
 };
 
 struct BackArgs {

@@ -49,6 +49,7 @@ cell_kernel(const __grid_constant__ MeshConst mc, const __grid_constant__ CellAr
     const bool vok = v < ar.nvec;
     const int flags = ar.flags;
     const bool hasph = mc.has_phase != 0;
+    const double isc = ar.in_scale > 0.0 ? ar.in_scale : 1.0;
 
     // ---- S1 gather
     {
@@ -72,6 +73,7 @@ cell_kernel(const __grid_constant__ MeshConst mc, const __grid_constant__ CellAr
                 }
             }
             if (flags & kScaleIn) val *= mc.im1[0][a] * mc.im1[1][b] * mc.im1[2][c];
+            if (sizeof(TT) == 4) val *= isc;                         // keep Z_k / s_k inside the FP32 range
             W[l * C + col] = (TT)val;
         }
     }
@@ -146,7 +148,7 @@ cell_kernel(const __grid_constant__ MeshConst mc, const __grid_constant__ CellAr
             const double mI = mab * mc.m1[2][k];
             const double imI = imab * mc.im1[2][k];
             const double sout = (flags & kSoutInvM) ? imI : 1.0;
-            double val = ar.cH * sout * (double)t[k];
+            double val = (sizeof(TT) == 4 ? ar.cH / isc : ar.cH) * sout * (double)t[k];
             if (hasph) {
                 const double other = __shfl_xor_sync(__activemask(), val, 1);
                 if (wx | wy | wz) {
@@ -222,7 +224,7 @@ proj_kernel(const NonlocalDev nl, const ProjArgs ar) {
         if (jj < it.count) {
             const long long I = nl.supp_node[soff + jj];
             x[jj] = __ldg(reinterpret_cast<const double2*>(ar.in) + (2 * I + s) * ar.ld_in + v);
-            if (ar.mass_u) { const double m = nl.supp_mass[soff + jj]; x[jj].x *= m; x[jj].y *= m; }
+            { const double m = (ar.mass_u ? nl.supp_mass[soff + jj] : 1.0) * ar.in_scale; x[jj].x *= m; x[jj].y *= m; }
         }
     }
     double* Crow = ar.C + (nl.c_off[it.atom] * (long long)ar.nvec + v) * 2;
@@ -332,7 +334,7 @@ proj_fast_kernel(const NonlocalDev nl, const ProjArgs ar) {
     if (threadIdx.x < kBig) {
         const int jj = threadIdx.x < it.count ? threadIdx.x : 0;
         nodes[threadIdx.x] = nl.supp_node[soff + jj];
-        mass[threadIdx.x] = ar.mass_u ? nl.supp_mass[soff + jj] : 1.0;
+        mass[threadIdx.x] = (ar.mass_u ? nl.supp_mass[soff + jj] : 1.0) * ar.in_scale;
     }
     __syncthreads();
     const int s = blockIdx.y & 1;

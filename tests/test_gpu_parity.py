@@ -363,3 +363,22 @@ def test_z_segments_of_more_than_one_cell(env, p, ncell, nvec):
         assert relerr(pb.gpu_filter(X, lam, 5, a, b, a0, B.FP32, B.RECUR_RESIDUAL), ref11) < TOL32
     finally:
         pb.close()
+
+
+@pytest.mark.parametrize("degree", [60, 500])
+def test_high_degree_scaled_recurrence_stays_accurate(env, degree):
+    """The in-place recurrence stores Z_k / s_k with s_{k+1} = -gamma_k s_{k-1}: at the paper's
+    q = 60 and far beyond, the scaling neither under- nor overflows and the result stays within 1e-11."""
+    _, fo, B = env
+    cfg = inp.tiny_config(ncell=2, p=4, L=4.0, kfrac=(0.25, 0, 0), nvec=8, natoms=1, nproj=8, ngauss=2)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, 8)
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref = fo.cheb_filter_residual(pb.oham, X, lam, degree, a, b, a0)
+        assert relerr(pb.gpu_filter(X, lam, degree, a, b, a0, B.FP64, B.RECUR_RESIDUAL), ref) < TOL64
+        assert relerr(pb.gpu_filter(X, None, degree, a, b, a0, B.FP64, B.RECUR_STANDARD), ref) < TOL64
+        assert relerr(pb.gpu_filter(X, lam, degree, a, b, a0, B.FP32, B.RECUR_RESIDUAL), ref) < TOL32
+    finally:
+        pb.close()
