@@ -86,6 +86,12 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
 }
+// the same with an L2 eviction-priority hint: the packed node fields are re-read by every vector chunk, so they are
+// loaded evict_last and stay in L2 while the multivectors stream through
+__device__ __forceinline__ void tma_load_2d_hint(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar, uint64_t policy) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)), "l"(policy) : "memory");
+}
 __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
@@ -655,6 +661,8 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
         // ================================ producer ================================
         if (lane == 0) {
             const int col0 = chunk * (C / 2);                     // doubles
+            uint64_t pol_last;
+            asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_last));
             for (int t = 0; t < T; ++t) {
                 const int s = t % STAGES;
                 const uint32_t par = (t / STAGES) & 1;
@@ -680,7 +688,7 @@ cell_march_kernel(const __grid_constant__ StepConst sc, const __grid_constant__ 
                 }
                 if (owned) {
                     if (ar.useR) tma_load_3d(st + Cfg::R_OFF, &mp.R, col0, xr, line, &full_bar[s]);
-                    tma_load_2d(st + Cfg::F_OFF, &mp.F, 4 * ex * P, line, &full_bar[s]);
+                    tma_load_2d_hint(st + Cfg::F_OFF, &mp.F, 4 * ex * P, line, &full_bar[s], pol_last);
                 }
             }
         }
