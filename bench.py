@@ -36,7 +36,7 @@ UNIT = "complex_DoF*vectors*degree/s"
 FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per cell-kernel launch from the committed `ncu --set full`
 # captures (profiles/r1_final_c1_ncu_full.md), keyed by (config, precision); None where no capture exists
-NCU_TRAFFIC = {(1, "fp64"): 1.847e9, (1, "fp32"): 1.850e9}
+NCU_TRAFFIC = {(1, "fp64"): 1.823e9, (1, "fp32"): 1.826e9}
 
 
 def measured_hbm_peak():
