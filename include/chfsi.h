@@ -122,14 +122,14 @@ chfsi_status chfsi_apply_H(const chfsi_mesh* mesh, chfsi_prec prec, int nvec, co
  * c = (a+b)/2, e = (b-a)/2, sigma_1 = e/(a0-c), sigma_{k+1} = 1/(2/sigma_1 - sigma_k).
  * recur STANDARD: eq. 10, Y_0 = X, Y_1 = sigma_1 (M^-1 H - c) X / e; lambda_host is ignored.
  * recur RESIDUAL: eq. 11 with D = M: R = H X - M X Lambda in FP64, Z_0 = 0, Z_1 = sigma_1 R / e,
- *   Lambda_k by the same recurrence in FP64 on the host, Y = D^-1 Z_m + X Lambda_m;
+ *   Lambda_k by the same recurrence in FP64 (one device thread per vector), Y = D^-1 Z_m + X Lambda_m;
  *   lambda_host: host, nvec Ritz values (any finite numbers are legal: with D = M the exact
  *   result does not depend on them).  With prec FP32 only the product H D^-1 Z_k is inexact;
  *   R, Z_k, Lambda_k and the four-term combination stay FP64.
  * The output is Y_m after m applications of H (m = 1 returns Y_1).
  * chunk = N_b > 0: vectors are processed in blocks of N_b columns ("N_b
  * wavefunctions"), chunk = 0: all at once.  Y may alias X exactly (same pointer and ld).
- * EINVAL: degree < 1, b <= a, a0 >= a, nvec < 1, ld < nvec, chunk < 0, chunk % 4 != 0 when
+ * EINVAL: degree < 1 or > 1024, b <= a, a0 >= a, nvec < 1, ld < nvec, chunk < 0, chunk % 4 != 0 when
  * 0 < chunk < nvec, NULL pointers, lambda_host NULL with RESIDUAL, work too small
  * or misaligned.  ESTATE: before chfsi_ham_set. */
 chfsi_status chfsi_cheb_filter(const chfsi_mesh* mesh, chfsi_prec prec, chfsi_recur recur,
