@@ -411,3 +411,117 @@ def test_nonlocal_block_elementwise_definition():
                             acc += P[ii, b] * D[2 * b + s, 2 * bp + t] * np.conj(P[jj, bp])
                     ref[2 * I + s, 2 * J + t] = m[I] * m[J] * acc
     assert np.max(np.abs(Hnl - ref)) < 1e-13 * np.max(np.abs(ref))
+
+
+# ------------------------------------------------------------------ pointwise local fields (eq. 12, O3)
+@pytest.mark.parametrize("nc,L,p,kfrac", [((3, 3, 3), (6.0, 6.0, 6.0), 3, (0.0, 0.0, 0.0)),
+                                          ((1, 3, 2), (2.0, 4.5, 3.0), 4, (0.25, 0.1, 0.0)),
+                                          ((2, 1, 1), (3.0, 2.0, 2.5), 2, (0.0, 0.0, 0.3))])
+def test_local_fields_act_pointwise_with_eq12_spin_blocks(nc, L, p, kfrac):
+    """With seeded NON-constant V, B and no projectors,  M^-1 H x - M^-1 H_0 x  (H_0: zero fields) must equal
+    [[V+Bz, Bx - i By], [Bx + i By, V - Bz]]_I x_I  node by node (eq. 12 spin blocks, pointwise
+    under GLL collocation, reading O3).  Pins WHICH node's field value stage (ii) of apply_H uses (a field
+    taken at a permuted node survives every constant-field pin and Hermiticity), and, on the meshes with a
+    single cell in a direction, the duplicate scatter of the potential term (np.add.at branch)."""
+    mesh = fo.Mesh(nc, L, p, kfrac)
+    rng = np.random.default_rng(77)
+    M = mesh.nnodes
+    V, Bx, By, Bz = (rng.uniform(-1.0, 1.0, M) for _ in range(4))
+    ham = fo.Hamiltonian(mesh, V, Bx, By, Bz)
+    ham0 = fo.Hamiltonian(mesh, None, None, None, None)
+    X = inp.make_vectors(M, 3, seed=9)
+    got = fo.apply_MinvH(ham, X) - fo.apply_MinvH(ham0, X)
+    up, dn = X[:, 0, :], X[:, 1, :]
+    ref = np.empty_like(X)
+    ref[:, 0, :] = (V + Bz)[:, None] * up + (Bx - 1j * By)[:, None] * dn
+    ref[:, 1, :] = (Bx + 1j * By)[:, None] * up + (V - Bz)[:, None] * dn
+    scale = np.max(np.abs(fo.apply_MinvH(ham0, X)))               # the difference cancels the kinetic term
+    assert np.max(np.abs(got - ref)) < 1e-13 * scale
+    # each field separately, so that a swap of two fields cannot cancel
+    for k, name in enumerate(["V", "Bx", "By", "Bz"]):
+        f = [None] * 4
+        f[k] = (V, Bx, By, Bz)[k]
+        hk = fo.Hamiltonian(mesh, *f)
+        gk = fo.apply_MinvH(hk, X) - fo.apply_MinvH(ham0, X)
+        fk = f[k][:, None]
+        rk = np.empty_like(X)
+        if name == "V":
+            rk[:, 0, :], rk[:, 1, :] = fk * up, fk * dn
+        elif name == "Bx":
+            rk[:, 0, :], rk[:, 1, :] = fk * dn, fk * up
+        elif name == "By":
+            rk[:, 0, :], rk[:, 1, :] = -1j * fk * dn, 1j * fk * up
+        else:
+            rk[:, 0, :], rk[:, 1, :] = fk * up, -fk * dn
+        assert np.max(np.abs(gk - rk)) < 1e-13 * scale, name
+
+
+# ------------------------------------------------------------------ node coordinates (PAPER.md:92 GLL nodes)
+def test_node_coords_closed_forms_and_quadrature_exactness():
+    """Mesh.node_coords: (i) closed forms -- p = 2: offsets {0, h/2}; p = 4: {0, h(1 - sqrt(3/7))/2, h/2,
+    h(1 + sqrt(3/7))/2} (the P1 golden nodes mapped to a cell); (ii) node ordering I = (iz N1y + iy) N1x + ix;
+    (iii) with the diagonal mass as weights the nodes integrate monomials of degree <= 2p-1 per direction
+    exactly:  sum_I m_I x_I^a y_I^b z_I^c = Lx^(a+1)/(a+1) ...  -- false for uniformly spaced nodes."""
+    m2 = fo.Mesh((2, 1, 1), (3.0, 1.0, 1.0), 2)
+    xyz = m2.node_coords()
+    assert xyz.shape == (m2.nnodes, 3)
+    assert np.allclose(xyz[:4, 0], [0.0, 0.75, 1.5, 2.25], atol=1e-15)        # h = 1.5: {0, h/2} per cell
+    m4 = fo.Mesh((1, 2, 1), (1.0, 4.0, 1.0), 4)
+    xyz = m4.node_coords()
+    h = 2.0
+    r = math.sqrt(3.0 / 7.0)
+    ref = np.array([0.0, h * (1 - r) / 2, h / 2, h * (1 + r) / 2])
+    ys = xyz[::4, 1][:8]                                                       # x fastest: stride N1x = 4 walks y
+    assert np.allclose(ys, np.concatenate([ref, h + ref]), atol=1e-15)
+    # ordering: x fastest, then y, then z
+    mesh = fo.Mesh((2, 3, 2), (3.0, 4.5, 2.0), 3)
+    xyz = mesh.node_coords()
+    n1x, n1y, n1z = mesh.n1
+    g = xyz.reshape(n1z, n1y, n1x, 3)
+    assert np.all(np.diff(g[0, 0, :, 0]) > 0) and np.all(g[:, :, 0, 0] == 0.0)
+    assert np.all(np.diff(g[0, :, 0, 1]) > 0) and np.all(g[:, 0, :, 1] == 0.0)
+    assert np.all(np.diff(g[:, 0, 0, 2]) > 0) and np.all(g[0, :, :, 2] == 0.0)
+    # quadrature exactness with m_I (degree <= 2p-1 = 5 per direction).  The mesh is periodic (the node at x = L
+    # is the node at x = 0), so the test functions vanish at both ends: f_a(t) = t^a (L - t), a >= 1.
+    Ls = mesh.L
+
+    def f(t, a, Ld):
+        return t ** a * (Ld - t)
+
+    def f_int(a, Ld):
+        return Ld ** (a + 2) / (a + 1) - Ld ** (a + 2) / (a + 2)
+
+    for (a, b, c) in [(1, 1, 1), (4, 1, 1), (1, 4, 1), (1, 1, 4), (2, 3, 1), (4, 4, 4), (3, 1, 2)]:
+        got = np.sum(mesh.mass * f(xyz[:, 0], a, Ls[0]) * f(xyz[:, 1], b, Ls[1]) * f(xyz[:, 2], c, Ls[2]))
+        exact = f_int(a, Ls[0]) * f_int(b, Ls[1]) * f_int(c, Ls[2])
+        assert abs(got - exact) < 1e-12 * exact, (a, b, c)
+    # ... and NOT beyond: degree 2p = 6 in one direction is not integrated exactly by (p+1)-point GLL
+    got = np.sum(mesh.mass * f(xyz[:, 0], 5, Ls[0]) * f(xyz[:, 1], 1, Ls[1]) * f(xyz[:, 2], 1, Ls[2]))
+    exact = f_int(5, Ls[0]) * f_int(1, Ls[1]) * f_int(1, Ls[2])
+    assert abs(got - exact) > 1e-7 * exact
+
+
+# ------------------------------------------------------------------ Algorithm 1 line 10
+def test_algorithm1_line10_bounds_update():
+    """Alg. 1 line 10: after each RR the filter is called with lambda_min <- lowest Ritz value,
+    lambda_T <- highest Ritz value of the block, lambda_max fixed.  Recorded through the filter_fn hook."""
+    cfg = inp.tiny_config(ncell=2, p=2, L=4.0, natoms=1, nproj=4)
+    mesh = _mesh(cfg)
+    ham, _ = _ham(cfg, mesh)
+    lam_exact, _, _ = _brute_force(ham)
+    calls = []
+
+    def spy(X, lam, m, a, bb, a0):
+        calls.append((np.array(lam), a, bb, a0))
+        return fo.cheb_filter_residual(ham, X, lam, m, a, bb, a0)
+
+    X0 = inp.make_vectors(mesh.nnodes, 6, seed=4)
+    b = lam_exact[-1] + 1.0
+    fo.subspace_iteration(ham, X0, degree=6, b=b, passes=3, tol=0.0, filter_fn=spy)
+    assert len(calls) == 3
+    for lam, a, bb, a0 in calls:
+        assert bb == b
+        assert a0 == lam[0] == np.min(lam)                 # lambda_min <- lambda_1
+        assert a == lam[-1] == np.max(lam)                 # lambda_T  <- lambda_N
+    # Ritz values decrease monotonically towards the exact ones from above
+    assert calls[2][0][0] <= calls[0][0][0] + 1e-12 and calls[2][0][0] >= lam_exact[0] - 1e-10
