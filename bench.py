@@ -1,22 +1,25 @@
 #!/usr/bin/env python
 """Benchmark of the Chebyshev-filter hot path (BASELINE.json metric) on B200.
 
-A "step" is one `chfsi_cheb_filter` call -- residual S0, m-1 recurrence steps, recover S7, i.e.
-every row of SURVEY.md §8(a) -- on BASELINE.json configs[1]: 8x8x8 periodic cells, side 16 Bohr,
-p = 6 (48^3 nodes, 221,184 complex DoF), 128 complex128 vectors, 8 atoms x 8 projectors,
-Chebyshev degree 20, FP64 throughout, the residual-based recurrence (eq. 11).
+A "step" is one `chfsi_cheb_filter` call -- residual S0, m-1 recurrence steps, recover S7, i.e. every row of
+SURVEY.md 8(a) -- over one block of synthetic vectors.  Default workload: BASELINE.json configs[3], the largest
+single-GPU configuration: 12x12x12 periodic cells, side 32 Bohr, p = 8 (96^3 nodes, 1.77M complex DoF), Bloch k-point
+(0.25,0,0) 2 pi/L, 216 atoms x 8 projectors, 1024 complex128 vectors processed in chunks of 256, Chebyshev degree 30,
+FP64 throughout (the paper's reference arithmetic), the residual-based recurrence (eq. 11).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1] [--prec fp64]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--prec fp64|fp32|fp32s]
 
-N > 1 (under torchrun): the filter shards over columns with no exchange (the paper's band
-partitioning in its n_r = 1 limit): every rank filters its own 128-vector block of
-the same mesh, value = all ranks' units / max-over-ranks time, scaling "weak".
-`--impl reference` times the CPU oracle (oracle/fe_oracle.py, as it stands) on a bounded sample.
+The JSON line also carries `all_configs`: one compact row per BASELINE config / precision (c0 latency; c1, c2, c3, the c4
+sweep: cell-kernel ms, its roofline fraction, whole-call fraction), measured in the same run (`--no-table` skips it).
+N > 1 (under torchrun): the filter shards over columns with no exchange (the paper's band partitioning in its n_r = 1
+limit): every rank filters its own block of the same mesh, value = all ranks' units / max-over-ranks
+time, scaling "weak".  `--impl reference` times the CPU oracle (oracle/fe_oracle.py, as it stands) on a bounded sample.
 Prints ONE JSON line.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -34,9 +37,9 @@ from paper_2605_30128_b200 import inputs as inp  # noqa: E402
 METRIC = "chebyshev_filter_throughput"
 UNIT = "complex_DoF*vectors*degree/s"
 FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per cell-kernel launch from the committed `ncu --set full`
-# captures (profiles/r1_final_c1_ncu_full.md), keyed by (config, precision); None where no capture exists
-NCU_TRAFFIC = {(1, "fp64"): 1.823e9, (1, "fp32"): 1.826e9}
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_cell_kernel_traffic.csv")
+DTYPE = {"fp64": "f64", "fp32": "f32 product / f64 storage and recurrence",
+         "fp32s": "f32 multivectors / f64 residual and Lambda_k"}
 
 
 def measured_hbm_peak():
@@ -45,6 +48,20 @@ def measured_hbm_peak():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(config, prec, nvec_launch):
+    """dram__bytes_read.sum + dram__bytes_write.sum per cell-kernel launch from the committed `ncu --set full` captures
+    (profiles/r2_cell_kernel_traffic.csv, written from the .ncu-rep files by the command in the .md beside it), keyed by
+    (config, precision, vectors per launch); None where no capture exists."""
+    try:
+        with open(TRAFFIC_CSV) as f:
+            for row in csv.DictReader(f):
+                if int(row["config"]) == config and row["prec"] == prec and int(row["nvec_per_launch"]) == nvec_launch:
+                    return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+    except Exception:
+        pass
+    return None
 
 
 class ClockSampler:
@@ -97,6 +114,15 @@ def units_per_step(cfg, nvec):
     return 2.0 * cfg.nnodes * nvec * cfg.degree
 
 
+def alg_bytes_per_unit(prec, recur="residual"):
+    """Algorithmic HBM bytes per unit of a recurrence step: eq. 11 reads Z_k and R and
+    read-modify-writes Z_{k-1} -> Z_{k+1}.  complex128: 16 + 16 + 32 = 64 B; complex64 iterates with R in FP64
+    ("only R and Lambda_k in FP64"): 8 + 16 + 16 = 40 B.  eq. 10: no R, 48 B."""
+    if recur != "residual":
+        return 48.0
+    return 40.0 if prec == "fp32s" else 64.0
+
+
 # --------------------------------------------------------------------------------------------
 def cpu_oracle_rate(cfg, ncols, repeat=1):
     """Oracle (eq. 11, FP64, as it stands) on `ncols` sampled columns of the workload; units/s."""
@@ -118,11 +144,17 @@ def cpu_oracle_rate(cfg, ncols, repeat=1):
     return units_per_step(cfg, ncols) / best, best, max(1, int(round(cpu_used)))
 
 
+def workload_name(args, cfg, nvec, chunk):
+    return (f"BASELINE configs[{args.config}] ({cfg.name}): {cfg.ncell}^3 cells, side {cfg.L} Bohr, p={cfg.p}, "
+            f"{2 * cfg.nnodes} complex DoF, kfrac {tuple(cfg.kfrac)}, {nvec} complex128 vectors in chunks of {chunk or nvec}, "
+            f"{cfg.natoms} atoms x {cfg.nproj} projectors, degree {cfg.degree}, recurrence {args.recur}, prec {args.prec}")
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    ncols = max(1, args.ref_cols // 4)      # each of the K + W steps is a bounded sample (~4 s): the run ends in about a minute
+    ncols = max(1, args.ref_cols // 2)      # each of the K + W steps is a bounded sample: the run ends within minutes
     times, cores = [], 1
     for i in range(args.warmup + args.steps):
         rate, dt, cores = cpu_oracle_rate(cfg, ncols)
@@ -135,9 +167,8 @@ def run_reference(args, cfg):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"BASELINE configs[{args.config}] ({cfg.name}): {cfg.ncell}^3 cells p={cfg.p}, "
-                               f"{cfg.nvec} vectors, degree {cfg.degree}, eq. 11", "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "config": {"workload": workload_name(args, cfg, cfg.nvec, cfg.chunk), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle (numpy, single process)", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -145,10 +176,231 @@ def run_reference(args, cfg):
 
 
 # --------------------------------------------------------------------------------------------
+class Workload:
+    """One mesh + Hamiltonian + device block, with the timing helpers used for the headline and for the table."""
+
+    def __init__(self, torch, B, cfg, prec_name, recur_name, nvec, device, seed, pb=None):
+        from paper_2605_30128_b200.harness import GpuProblem
+        self.torch, self.B, self.cfg = torch, B, cfg
+        self.prec = B.PREC[prec_name]
+        self.recur = B.RECUR_RESIDUAL if recur_name == "residual" else B.RECUR_STANDARD
+        self.nvec = nvec
+        self.chunk = cfg.chunk if (cfg.chunk and cfg.chunk < nvec) else (256 if nvec > 512 else 0)
+        self.own_pb = pb is None
+        self.pb = pb if pb is not None else GpuProblem(cfg, seed=0, device=device)
+        dev = f"cuda:{device}"
+        g = torch.Generator(device=dev); g.manual_seed(seed)
+        self.X = torch.empty((cfg.nnodes, 2, nvec), dtype=torch.complex128, device=dev)
+        Xr = torch.view_as_real(self.X)
+        for j0 in range(0, nvec, 64):                      # filled in slabs: no full-size temporaries
+            j1 = min(nvec, j0 + 64)
+            Xr[:, :, j0:j1, :] = torch.rand((cfg.nnodes, 2, j1 - j0, 2), generator=g, device=dev, dtype=torch.float64) * 2 - 1
+        self.Y = torch.empty_like(self.X)
+        self.a0, self.b = self.pb.lanczos_bounds(10)
+        self.a = self.a0 + 0.1 * (self.b - self.a0)
+        self.lam = self.pb.rayleigh_quotients(self.X) if self.recur == B.RECUR_RESIDUAL else None
+        self.work = self.pb.work(self.prec, self.recur, self.chunk if self.chunk else nvec)
+        self.stream = torch.cuda.current_stream()
+
+    def step(self):
+        self.B.chfsi_cheb_filter(self.pb.mesh, self.prec, self.recur, self.cfg.degree, self.a, self.b, self.a0, self.X,
+                                 self.lam, self.Y, self.work, chunk=self.chunk, stream=self.stream)
+
+    def time_steps(self, steps, warmup, barrier=None):
+        torch = self.torch
+        for _ in range(warmup):
+            self.step()
+        (barrier or torch.cuda.synchronize)()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        ev[0].record(self.stream)
+        for i in range(steps):
+            self.step()
+            ev[i + 1].record(self.stream)
+        (barrier or torch.cuda.synchronize)()
+        per = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+        return ev[0].elapsed_time(ev[steps]), per
+
+    def cell_profile(self, nsteps):
+        """Cell-kernel launches of `nsteps` filter calls, timed with CUDA events on the launching stream by the library
+        (the nonlocal kernels then run on the same stream instead of the forked side stream)."""
+        B = self.B
+        B.chfsi_profile_enable(self.pb.mesh, True)
+        for _ in range(nsteps):
+            self.step()
+        cell_ms, cell_n, cell_bytes = B.chfsi_profile_read(self.pb.mesh)
+        B.chfsi_profile_enable(self.pb.mesh, False)
+        return cell_ms, cell_n, cell_bytes
+
+    def close(self):
+        self.X = self.Y = self.work = None
+        self.pb._work = {}
+        if self.own_pb:
+            self.pb.close()
+        self.torch.cuda.empty_cache()
+
+
+def config_row(torch, B, cfg_id, prec, nvec, device, peak, steps=2, warmup=1, pb=None):
+    """One row of the all-config table."""
+    cfg = inp.CONFIGS[cfg_id]
+    w = Workload(torch, B, cfg, prec, "residual", nvec, device, 4321, pb=pb)
+    try:
+        ms_total, _ = w.time_steps(steps, warmup)
+        ms_step = ms_total / steps
+        cell_ms, cell_n, cell_bytes = w.cell_profile(1)
+        bpu = alg_bytes_per_unit(prec)
+        ups = units_per_step(cfg, nvec) / (ms_step * 1e-3)
+        return {"config": cfg_id, "prec": prec, "nvec": nvec, "chunk": w.chunk or nvec, "filter_ms": round(ms_step, 4),
+                "units_per_s": float(f"{ups:.4g}"), "cell_ms": round(cell_ms / cell_n, 5),
+                "cell_frac": round(cell_bytes / (cell_ms * 1e-3) / 1e9 / peak, 4),
+                "whole_frac": round(ups * bpu / (peak * 1e9), 4), "alg_bytes_per_unit": bpu}
+    finally:
+        w.close()
+
+
+def all_configs_table(torch, B, device, peak):
+    """c0 (latency, also through a CUDA graph), c1, c3 (one chunk) and the c4 sweep (c2 = its 512-vector rows) in every
+    built precision."""
+    from paper_2605_30128_b200.harness import GpuProblem
+    rows = []
+    # c0: launch / latency bound -- time only, plain launch and graph replay
+    cfg0 = inp.CONFIGS[0]
+    w = Workload(torch, B, cfg0, "fp64", "residual", cfg0.nvec, device, 4321)
+    try:
+        ms_total, _ = w.time_steps(20, 5)
+        row = {"config": 0, "prec": "fp64", "nvec": cfg0.nvec, "filter_ms": round(ms_total / 20, 4),
+               "note": "launch/latency bound: time only"}
+        try:
+            s = torch.cuda.Stream()
+            s.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(s):
+                w.stream = s
+                w.step(); s.synchronize()
+                gr = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gr, stream=s):
+                    w.step()
+                for _ in range(3):
+                    gr.replay()
+                s.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(s)
+                for _ in range(20):
+                    gr.replay()
+                e1.record(s); s.synchronize()
+                row["filter_ms_cuda_graph"] = round(e0.elapsed_time(e1) / 20, 4)
+        except Exception as ex:                                   # graph capture is a convenience of the harness
+            row["filter_ms_cuda_graph"] = None
+            row["graph_error"] = str(ex)[:160]
+        rows.append(row)
+    finally:
+        w.close()
+    for cfg_id, precs, nvecs in [(1, ["fp64", "fp32", "fp32s"], [128]), (3, ["fp64", "fp32", "fp32s"], [256]),
+                                 (4, ["fp64", "fp32", "fp32s"], [64, 128, 256, 512, 1024])]:
+        cfg = inp.CONFIGS[cfg_id]
+        pb = GpuProblem(cfg, seed=0, device=device)
+        try:
+            for nvec in nvecs:
+                for prec in precs:
+                    row = config_row(torch, B, cfg_id, prec, nvec, device, peak, pb=pb)
+                    if cfg_id == 4 and nvec == 512:
+                        row["also"] = "configs[2] (same mesh, 512 vectors, degree 24)"
+                    if cfg_id == 3:
+                        row["note"] = "one 256-vector chunk of configs[3]; the headline line runs all four"
+                    rows.append(row)
+        finally:
+            pb.close()
+    return rows
+
+
+# --------------------------------------------------------------------------------------------
+def run_e2e(torch, B, w, world, dist, barrier, n_steps):
+    """The same filter through the C ABI with HOST buffers: every step uploads all of X from pinned host memory and
+    downloads all of Y into pinned host memory inside the timed region.  The block moves through a FIXED ring of pinned
+    slots (node ranges of a chunk are contiguous byte ranges, so every copy is a plain cudaMemcpyAsync); upload of chunk
+    c+1 and download of chunk c-1 overlap the filter call on chunk c (three streams)."""
+    cfg, nvec = w.cfg, w.nvec
+    chunk = w.chunk or nvec
+    nchunks = (nvec + chunk - 1) // chunk
+    dev = w.X.device
+    row_bytes = 2 * chunk * 16                                  # one node of a chunk
+    slot_nodes = max(1, min(cfg.nnodes, int(1.0e9 // row_bytes)))    # ~1 GB slots
+    npieces = (cfg.nnodes + slot_nodes - 1) // slot_nodes
+    NSLOT = 4
+    hin = [torch.empty((slot_nodes, 2, chunk), dtype=torch.complex128, pin_memory=True) for _ in range(NSLOT)]
+    hout = [torch.empty((slot_nodes, 2, chunk), dtype=torch.complex128, pin_memory=True) for _ in range(NSLOT)]
+    hin[0].copy_(w.X[:slot_nodes, :, :chunk])
+    for h in hin[1:]:
+        h.copy_(hin[0])
+    Xd = [torch.empty((cfg.nnodes, 2, chunk), dtype=torch.complex128, device=dev) for _ in range(2)]
+    Yd = [torch.empty((cfg.nnodes, 2, chunk), dtype=torch.complex128, device=dev) for _ in range(2)]
+    work = w.pb.work(w.prec, w.recur, chunk)
+    lam = w.lam
+    s_in, s_out, stream = torch.cuda.Stream(), torch.cuda.Stream(), w.stream
+    ev_in = [torch.cuda.Event() for _ in range(2)]
+    ev_c = [torch.cuda.Event() for _ in range(2)]
+    ev_out = [torch.cuda.Event() for _ in range(2)]
+    state = {"piece": 0}
+
+    def upload(c):
+        with torch.cuda.stream(s_in):
+            s_in.wait_event(ev_c[c % 2])                          # the filter call that read this buffer two chunks ago
+            for p0 in range(npieces):
+                n0, n1 = p0 * slot_nodes, min(cfg.nnodes, (p0 + 1) * slot_nodes)
+                Xd[c % 2][n0:n1].copy_(hin[state["piece"] % NSLOT][: n1 - n0], non_blocking=True)
+                state["piece"] += 1
+            ev_in[c % 2].record(s_in)
+
+    def download(c):
+        with torch.cuda.stream(s_out):
+            s_out.wait_event(ev_c[c % 2])
+            for p0 in range(npieces):
+                n0, n1 = p0 * slot_nodes, min(cfg.nnodes, (p0 + 1) * slot_nodes)
+                hout[p0 % NSLOT][: n1 - n0].copy_(Yd[c % 2][n0:n1], non_blocking=True)
+            ev_out[c % 2].record(s_out)
+
+    def e2e_step():
+        upload(0)
+        for c in range(nchunks):
+            if c + 1 < nchunks:
+                upload(c + 1)
+            stream.wait_event(ev_in[c % 2])
+            stream.wait_event(ev_out[c % 2])                      # Yd[c % 2] was downloaded (two chunks ago)
+            j0 = c * chunk
+            nb = min(chunk, nvec - j0)
+            B.chfsi_cheb_filter(w.pb.mesh, w.prec, w.recur, cfg.degree, w.a, w.b, w.a0, Xd[c % 2],
+                                None if lam is None else lam[j0:j0 + nb], Yd[c % 2], work, stream=stream, nvec=nb)
+            ev_c[c % 2].record(stream)
+            download(c)
+
+    for e in ev_c + ev_out:
+        e.record(stream)
+    e2e_step(); barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s_in.wait_stream(stream); s_out.wait_stream(stream)
+    e0.record(s_in)
+    for _ in range(n_steps):
+        e2e_step()
+        s_in.wait_stream(s_out)                                   # the next step's uploads start after this step's downloads were queued
+    s_out.wait_stream(stream); s_out.wait_stream(s_in)
+    e1.record(s_out)
+    barrier()
+    ms_e2e = e0.elapsed_time(e1) / n_steps
+    if dist is not None:
+        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    nbytes = cfg.nnodes * 2 * nvec * 16
+    del Xd, Yd, hin, hout
+    torch.cuda.empty_cache()
+    return {"value": world * units_per_step(cfg, nvec) / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+            "d2h_bytes_per_step": nbytes, "ms_per_step": ms_e2e,
+            "how": f"{nchunks} chunk(s) of {chunk} vectors; each chunk crosses PCIe as {npieces} contiguous node ranges through a fixed "
+                   f"ring of {NSLOT}+{NSLOT} pinned slots of {slot_nodes * row_bytes / 1e9:.2f} GB; upload, filter and download "
+                   f"pipelined on three streams"}
+
+
 def run_ours(args, cfg):
     import torch
     from paper_2605_30128_b200 import binding as B
-    from paper_2605_30128_b200.harness import GpuProblem
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -166,153 +418,81 @@ def run_ours(args, cfg):
     if dist is not None:
         dist.barrier()
     B.lib()
-    dev = f"cuda:{local}"
-    prec = B.PREC[args.prec]
-    recur = B.RECUR_RESIDUAL if args.recur == "residual" else B.RECUR_STANDARD
     nvec = args.nvec or cfg.nvec
-    chunk = cfg.chunk if (cfg.chunk and cfg.chunk < nvec) else 0
-
-    pb = GpuProblem(cfg, seed=0, device=local)
-    g = torch.Generator(device=dev); g.manual_seed(1234 + rank)
-    shape = (cfg.nnodes, 2, nvec)
-    X = torch.complex(torch.rand(shape, generator=g, device=dev, dtype=torch.float64) * 2 - 1,
-                      torch.rand(shape, generator=g, device=dev, dtype=torch.float64) * 2 - 1)
-    Y = torch.empty_like(X)
-    a0, b = pb.lanczos_bounds(10)
-    a = a0 + 0.1 * (b - a0)
-    lam = pb.rayleigh_quotients(X) if recur == B.RECUR_RESIDUAL else None
-    work = pb.work(prec, recur, chunk if chunk else nvec)
-    stream = torch.cuda.current_stream()
-
-    def step():
-        B.chfsi_cheb_filter(pb.mesh, prec, recur, cfg.degree, a, b, a0, X, lam, Y, work, chunk=chunk, stream=stream)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step()
+    w = Workload(torch, B, cfg, args.prec, args.recur, nvec, local, 1234 + rank)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
-        step()
-    e1.record(stream)
-    barrier()
-    ms_total = e0.elapsed_time(e1)
+    ms_total, per_step = w.time_steps(args.steps, args.warmup, barrier)
     launches = B.chfsi_last_launch_count() * args.steps
     clocks = sampler.stop() if rank == 0 else None
+    dev = f"cuda:{local}"
     if dist is not None:
         t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_total = float(t.item())
     ms_step = ms_total / args.steps
     value = world * units_per_step(cfg, nvec) / (ms_step * 1e-3)
-    assert bool(torch.isfinite(Y.real).all()), "filter output is not finite"
+    assert bool(torch.isfinite(torch.view_as_real(w.Y[:, :, :8])).all()), "filter output is not finite"
 
     # ---- roofline of the dominant kernel (cell kernel), timed live with CUDA events on its stream
-    B.chfsi_profile_enable(pb.mesh, True)
-    for _ in range(max(1, min(3, args.steps))):
-        step()
-    cell_ms, cell_n, cell_bytes = B.chfsi_profile_read(pb.mesh)
-    B.chfsi_profile_enable(pb.mesh, False)
+    big = units_per_step(cfg, nvec) > 5e9
+    steps_prof = 1 if big else max(1, min(3, args.steps))
+    cell_ms, cell_n, cell_bytes = w.cell_profile(steps_prof)
     peak, peak_src = measured_hbm_peak()
     achieved = cell_bytes / (cell_ms * 1e-3) / 1e9
-    steps_prof = max(1, min(3, args.steps))
-    roofline = {"bound": "hbm", "kernel": "cell_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": args.traffic if args.traffic is not None else (NCU_TRAFFIC.get((args.config, args.prec)) if nvec == cfg.nvec else None),
+    bpu = alg_bytes_per_unit(args.prec, args.recur)
+    chunk_used = w.chunk
+    roofline = {"bound": "hbm", "kernel": "cell kernel (gather + sum-factorised Laplacian + assembly + pointwise + update)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": args.traffic if args.traffic is not None else ncu_traffic(args.config, args.prec, chunk_used or nvec),
                 "avg_launch_ms": cell_ms / cell_n, "launches_per_step": cell_n // steps_prof,
                 "share_of_step": (cell_ms / steps_prof) / ms_step,
-                "alg_bytes_per_launch": cell_bytes / cell_n}
+                "alg_bytes_per_launch": cell_bytes / cell_n,
+                "note": "launches timed with the nonlocal kernels on the same stream (the headline run forks them to a side stream)"}
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
-    # (X and Y themselves are the device buffers: the host copy of X is what was uploaded before)
-    nbytes = X.numel() * 16
-    if args.no_e2e or nbytes > args.e2e_max_gb * 1e9:
-        e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
-               "skipped": f"host staging of 2 x {nbytes / 1e9:.1f} GB pinned buffers not attempted (--e2e-max-gb)"}
+    if args.no_e2e:
+        nbytes = cfg.nnodes * 2 * nvec * 16
+        e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "skipped": "--no-e2e"}
     else:
-        # The host holds the block as `nblk` band blocks (column groups, each [M, 2, nvec/nblk] contiguous and
-        # pinned); block i+1 is uploaded and block i-1 downloaded while block i is filtered (three streams).
-        nblk = 4 if (nvec % 4 == 0 and nvec >= 64) else 1
-        cw = nvec // nblk
-        bshape = (cfg.nnodes, 2, cw)
-        Xh = [torch.empty(bshape, dtype=torch.complex128, pin_memory=True) for _ in range(nblk)]
-        Yh = [torch.empty(bshape, dtype=torch.complex128, pin_memory=True) for _ in range(nblk)]
-        for i in range(nblk):
-            Xh[i].copy_(X[:, :, i * cw:(i + 1) * cw])
-        Xd = [torch.empty(bshape, dtype=torch.complex128, device=dev) for _ in range(nblk)]
-        Yd = [torch.empty(bshape, dtype=torch.complex128, device=dev) for _ in range(nblk)]
-        lam_b = [None if lam is None else lam[i * cw:(i + 1) * cw] for i in range(nblk)]
-        work_b = pb.work(prec, recur, cw)
-        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
-        ev_in = [torch.cuda.Event() for _ in range(nblk)]
-        ev_c = [torch.cuda.Event() for _ in range(nblk)]
+        e2e = run_e2e(torch, B, w, world, dist, barrier, max(1, min(args.steps, 2 if big else 5)))
 
-        def e2e_step():
-            for i in range(nblk):
-                with torch.cuda.stream(s_in):
-                    Xd[i].copy_(Xh[i], non_blocking=True)
-                    ev_in[i].record(s_in)
-                stream.wait_event(ev_in[i])
-                B.chfsi_cheb_filter(pb.mesh, prec, recur, cfg.degree, a, b, a0, Xd[i], lam_b[i], Yd[i], work_b,
-                                    stream=stream)
-                ev_c[i].record(stream)
-                s_out.wait_event(ev_c[i])
-                with torch.cuda.stream(s_out):
-                    Yh[i].copy_(Yd[i], non_blocking=True)
-
-        e2e_step(); barrier()
-        n_e2e = max(1, min(args.steps, 5))
-        s_in.wait_stream(stream); s_out.wait_stream(stream)
-        e0.record(s_in)
-        for _ in range(n_e2e):
-            e2e_step()
-            s_in.wait_stream(s_out)          # the next step's uploads start after this step's downloads were queued
-        s_out.wait_stream(stream); s_out.wait_stream(s_in)
-        e1.record(s_out)
-        barrier()
-        ms_e2e = e0.elapsed_time(e1) / n_e2e
-        if dist is not None:
-            t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e2e = float(t.item())
-        e2e = {"value": world * units_per_step(cfg, nvec) / (ms_e2e * 1e-3), "unit": UNIT,
-               "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "ms_per_step": ms_e2e,
-               "how": f"{nblk} pinned host band blocks of {cw} vectors; upload, filter and download pipelined on three streams"}
+    w.close()
+    table = None
+    if rank == 0 and world == 1 and not args.no_table:
+        table = all_configs_table(torch, B, local, peak)
 
     # ---- CPU oracle baseline on a bounded sample (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         rate, dt, cores = cpu_oracle_rate(cfg, args.ref_cols)
-        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle (numpy, single process)", "seconds": dt,
                "sample": f"{args.ref_cols} of {cfg.nvec} columns of {cfg.name}, full degree {cfg.degree}, eq. 11 FP64"}
 
     if rank == 0:
+        nbytes = cfg.nnodes * 2 * nvec * 16
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64" if args.prec == "fp64" else "f32 product / f64 recurrence",
-            "data": "synthetic",
-            "config": {"workload": f"BASELINE configs[{args.config}] ({cfg.name}): {cfg.ncell}^3 cells, side {cfg.L} Bohr, "
-                                   f"p={cfg.p}, {2 * cfg.nnodes} complex DoF, {nvec} complex128 vectors, "
-                                   f"{cfg.natoms} atoms x {cfg.nproj} projectors, degree {cfg.degree}, "
-                                   f"recurrence {args.recur}, prec {args.prec}, chunk {chunk or nvec}",
+            "warmup": args.warmup, "ms_per_step": ms_step, "median_ms_per_step": float(np.median(per_step)),
+            "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": DTYPE[args.prec], "data": "synthetic",
+            "config": {"workload": workload_name(args, cfg, nvec, chunk_used),
                        "l2": f"inputs larger than L2 (each multivector {nbytes / 1e6:.0f} MB vs 126 MB L2)",
                        "parallelism": "columns sharded, no exchange" if world > 1 else "1 GPU"},
             "units_per_step": units_per_step(cfg, nvec), "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu,
             "gpu_launches": int(launches), "clocks": clocks,
-            "roofline_whole_filter": {"alg_bytes_per_unit": 64 if recur == B.RECUR_RESIDUAL else 48,
-                                      "frac_of_hbm_peak": value / world * (64 if recur == B.RECUR_RESIDUAL else 48) / (peak * 1e9)},
+            "roofline_whole_filter": {"alg_bytes_per_unit": bpu, "frac_of_hbm_peak": value / world * bpu / (peak * 1e9)},
+            "all_configs": table,
         }
         print(json.dumps(line))
-    pb.close()
     if dist is not None:
         dist.destroy_process_group()
 
@@ -320,26 +500,26 @@ def run_ours(args, cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--prec", default=None, choices=["fp64", "fp32"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--prec", default=None, choices=["fp64", "fp32", "fp32s"])
     ap.add_argument("--recur", default="residual", choices=["residual", "standard"])
     ap.add_argument("--nvec", type=int, default=0)
     ap.add_argument("--ref-cols", type=int, default=0, help="columns in the CPU-oracle sample")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--e2e-max-gb", type=float, default=8.0, help="skip the host-staged e2e leg above this block size")
+    ap.add_argument("--no-table", action="store_true", help="skip the all-config table")
     ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per cell-kernel launch from the committed ncu capture (profiles/)")
+                    help="dram bytes per cell-kernel launch (overrides the value read from profiles/)")
     args = ap.parse_args()
     cfg = inp.CONFIGS[args.config]
     if args.ref_cols <= 0:
-        # about 10-20 s of oracle time: ~8.5e6 units/s on one host core
-        args.ref_cols = max(1, min(cfg.nvec, int(round(1.2e8 / (2.0 * cfg.nnodes * cfg.degree)))))
+        # about 10-20 s of oracle time: ~1e7 units/s on one host core
+        args.ref_cols = max(1, min(cfg.nvec, int(round(1.5e8 / (2.0 * cfg.nnodes * cfg.degree)))))
     if args.prec is None:
-        args.prec = cfg.prec if args.config != 1 else "fp64"
+        args.prec = "fp64"            # the paper's reference arithmetic; --prec fp32 / fp32s select the inexact modes
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

@@ -53,10 +53,15 @@ typedef enum {
 /* Precision of the H.X product inside the recurrence ("FP32 or TF32").
  * The recurrence itself, the residual R and Lambda_k are always FP64. */
 typedef enum {
-    CHFSI_FP64 = 0,
-    CHFSI_FP32 = 1,
+    CHFSI_FP64 = 0,          /* everything FP64 */
+    CHFSI_FP32 = 1,          /* H.X product in FP32 on fl32(Z_k); Z_k, R, Lambda_k and the recurrence stored/combined in FP64 */
     CHFSI_TF32 = 2,          /* reserved: returns CHFSI_EUNSUPPORTED in this build */
-    CHFSI_TF32X3 = 3         /* reserved: returns CHFSI_EUNSUPPORTED in this build */
+    CHFSI_TF32X3 = 3,        /* reserved: returns CHFSI_EUNSUPPORTED in this build */
+    CHFSI_FP32_STORED = 4    /* the paper's layout: the multivectors Z_k themselves are complex64 inside the
+                                filter ("extraction, scatter/gather, and assembly kernels ... operate on FP32 multivectors,
+                                halving global memory traffic"), FP32 arithmetic; "only the eigenproblem residual R and the
+                                eigenvalue recurrence Lambda_k are retained in FP64", as are S0 and the recover step S7.
+                                chfsi_cheb_filter with CHFSI_RECUR_RESIDUAL and even p only (EUNSUPPORTED otherwise). */
 } chfsi_prec;
 
 typedef enum {

@@ -16,9 +16,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libchfsi.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED = range(6)
-FP64, FP32, TF32, TF32X3 = range(4)
+FP64, FP32, TF32, TF32X3, FP32_STORED = range(5)
 RECUR_STANDARD, RECUR_RESIDUAL = 0, 1
-PREC = {"fp64": FP64, "fp32": FP32, "tf32": TF32, "tf32x3": TF32X3}
+PREC = {"fp64": FP64, "fp32": FP32, "tf32": TF32, "tf32x3": TF32X3, "fp32s": FP32_STORED}
 
 EXPORTS = [
     "chfsi_mesh_create", "chfsi_mesh_destroy", "chfsi_mesh_num_nodes", "chfsi_mesh_node_coords",

@@ -10,8 +10,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libchfsi.so")
-SOURCES = ["chfsi.cu", "kernels.cu", "cell_march.cu"]
-HEADERS = [os.path.join(CSRC, "chfsi_internal.h"), os.path.join(ROOT, "include", "chfsi.h")]
+SOURCES = ["chfsi.cu", "kernels.cu", "cell_march.cu", "cell_xyz.cu"]
+HEADERS = [os.path.join(CSRC, "chfsi_internal.h"), os.path.join(CSRC, "tma_util.cuh"), os.path.join(ROOT, "include", "chfsi.h")]
 
 
 def _nvcc() -> str:

@@ -108,17 +108,22 @@ static size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 
 // workspace layout: [coef table][Cbuf][nbuf multivector buffers]
 struct WorkLayout {
-    size_t hdr_bytes, coef_bytes, c_bytes, buf_bytes, total;
+    size_t hdr_bytes, coef_bytes, c_bytes, buf_bytes, zbuf_bytes, total;
     int nbuf;
+    long long ldz;      // leading dimension of the two iterate buffers (complex elements)
 };
-static WorkLayout work_layout(const chfsi_mesh* m, chfsi_recur recur, int chunk, int degree_cap) {
+static WorkLayout work_layout(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur recur, int chunk, int degree_cap) {
     WorkLayout wl;
     wl.nbuf = recur == CHFSI_RECUR_RESIDUAL ? 3 : 1;
     wl.hdr_bytes = align256((size_t)(4 + 9 * (degree_cap + 2) + chunk) * sizeof(double));
     wl.coef_bytes = align256((size_t)(degree_cap + 2) * 2 * chunk * sizeof(double));
     wl.c_bytes = 2 * align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * chunk * 16);   // C and G
     wl.buf_bytes = align256((size_t)2 * m->nnodes * chunk * 16);
-    wl.total = wl.hdr_bytes + wl.coef_bytes + wl.c_bytes + wl.nbuf * wl.buf_bytes;
+    // FP32-stored multivectors: R stays complex128, the two iterate buffers are complex64 with an even leading
+    // dimension (16-byte row pitch for TMA)
+    wl.ldz = prec == CHFSI_FP32_STORED ? ((chunk + 1) & ~1) : chunk;
+    wl.zbuf_bytes = prec == CHFSI_FP32_STORED ? align256((size_t)2 * m->nnodes * wl.ldz * 8) : wl.buf_bytes;
+    wl.total = wl.hdr_bytes + wl.coef_bytes + wl.c_bytes + wl.buf_bytes + (wl.nbuf - 1) * wl.zbuf_bytes;
     return wl;
 }
 constexpr int kDegreeCap = 1024;   // coefficient table is sized for degree <= kDegreeCap
@@ -226,6 +231,8 @@ chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
         if (m->ev_proj) cudaEventDestroy(m->ev_proj);
         if (m->ev_back) cudaEventDestroy(m->ev_back);
         if (m->side) cudaStreamDestroy(m->side);
+        for (cudaEvent_t e : m->stage_ev) if (e) cudaEventDestroy(e);
+        if (m->h_stage) cudaFreeHost(m->h_stage);
         cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF);
         free_nonlocal(m->nl);
     }
@@ -311,9 +318,11 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
         if (m->dF == nullptr) CU(cudaMalloc(reinterpret_cast<void**>(&m->dF), (size_t)M * 32));
         CU(cudaMemcpy(m->dF, F.data(), (size_t)M * 32, cudaMemcpyHostToDevice));
     }
-    // ---- nonlocal tables
-    free_nonlocal(m->nl);
-    NonlocalDev& nl = m->nl;
+    // ---- nonlocal tables: built in a local object and swapped in only when every upload has succeeded, so that a failed
+    // re-set never leaves the mesh with half-built tables (the mesh is marked unset meanwhile)
+    m->ham_set = false;
+    NonlocalDev nl;
+    struct NlGuard { NonlocalDev* p; ~NlGuard() { if (p) free_nonlocal(*p); } } nlguard{&nl};
     nl.natoms = natoms; nl.nnz = nnz; nl.max_nproj = max_np; nl.crows = crows;
     if (natoms > 0 && nnz > 0) {
         std::vector<ProjItem> items;
@@ -359,6 +368,15 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
         CU(upload(&nl.P32, P32));
         CU(upload(&nl.D64, D64));
     }
+    free_nonlocal(m->nl);
+    m->nl = nl;
+    nlguard.p = nullptr;
+    if (!m->h_stage) {   // pinned staging ring of the filter's coefficient program (setup call: allocation is allowed here)
+        m->stage_slot_doubles = 4 + 9 * (size_t)(kDegreeCap + 2) + chfsi_mesh::kStageLambda;
+        CU(cudaHostAlloc(reinterpret_cast<void**>(&m->h_stage), chfsi_mesh::kStageSlots * m->stage_slot_doubles * sizeof(double),
+                         cudaHostAllocDefault));
+        for (int i = 0; i < chfsi_mesh::kStageSlots; ++i) CU(cudaEventCreateWithFlags(&m->stage_ev[i], cudaEventDisableTiming));
+    }
     if (!m->side) {   // side stream of the projector back-pass (setup call: allocation is allowed here)
         int lo = 0, hi = 0;
         CU(cudaDeviceGetStreamPriorityRange(&lo, &hi));              // lo = lowest priority (largest number)
@@ -376,7 +394,9 @@ chfsi_status chfsi_workspace_bytes(const chfsi_mesh* m, chfsi_prec prec, chfsi_r
     if (chunk < 1) return fail(CHFSI_EINVAL, "workspace_bytes: chunk must be >= 1");
     if (recur != CHFSI_RECUR_STANDARD && recur != CHFSI_RECUR_RESIDUAL) return fail(CHFSI_EINVAL, "workspace_bytes: bad recur");
     if (!cell_supported(m->p, prec)) return fail(CHFSI_EUNSUPPORTED, "workspace_bytes: precision not built");
-    *bytes = work_layout(m, recur, chunk, kDegreeCap).total;
+    if (prec == CHFSI_FP32_STORED && recur != CHFSI_RECUR_RESIDUAL)
+        return fail(CHFSI_EUNSUPPORTED, "workspace_bytes: FP32-stored multivectors need the residual recurrence (eq. 11)");
+    *bytes = work_layout(m, prec, recur, chunk, kDegreeCap).total;
     return CHFSI_OK;
 }
 
@@ -390,8 +410,8 @@ static chfsi_status accumulate_H(const chfsi_mesh* m, chfsi_prec prec, const Cel
     double* Gbuf = reinterpret_cast<double*>(reinterpret_cast<char*>(Cbuf) +
                                              align256((size_t)m->nl.crows * ca.nvec * 16));
     const double isc = (prec == CHFSI_FP32 && ca.in_scale > 0.0) ? ca.in_scale : 1.0;
-    ProjArgs pa{ca.in, ca.ld_in, Cbuf, ca.nvec, (ca.flags & kScaleIn) ? 0 : 1, isc};
-    BackArgs ba{Cbuf, Gbuf, ca.out, ca.ld_out, ca.cH / isc, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0};
+    ProjArgs pa{ca.in, ca.ld_in, Cbuf, ca.nvec, (ca.flags & kScaleIn) ? 0 : 1, isc, ca.store_f32};
+    BackArgs ba{Cbuf, Gbuf, ca.out, ca.ld_out, ca.cH / isc, ca.nvec, (ca.flags & kSoutInvM) ? 1 : 0, ca.store_f32};
     if (fork) {
         // The nonlocal term (zero C, project, back-project) depends on `in` only and, like the cell kernel, only
         // accumulates into `out` (RED): it runs on the mesh's low-priority stream beside the cell kernel and takes
@@ -399,12 +419,15 @@ static chfsi_status accumulate_H(const chfsi_mesh* m, chfsi_prec prec, const Cel
         CU(cudaEventRecord(m->ev_proj, st));
         CU(launch_cell(m, prec, ca, st));                            // first, so that its CTAs take the SMs
         CU(cudaStreamWaitEvent(m->side, m->ev_proj, 0));
-        CU(cudaMemsetAsync(Cbuf, 0, (size_t)m->nl.crows * ca.nvec * 16, m->side));
+        // from here on the side stream has been forked: whatever fails, it is joined back into the caller's stream
+        cudaError_t e = cudaMemsetAsync(Cbuf, 0, (size_t)m->nl.crows * ca.nvec * 16, m->side);
         count_launch();
-        CU(launch_proj(m, prec, pa, m->side));
-        CU(launch_back(m, prec, ba, m->side));
-        CU(cudaEventRecord(m->ev_back, m->side));
-        CU(cudaStreamWaitEvent(st, m->ev_back, 0));
+        if (e == cudaSuccess) e = launch_proj(m, prec, pa, m->side);
+        if (e == cudaSuccess) e = launch_back(m, prec, ba, m->side);
+        cudaError_t ej = cudaEventRecord(m->ev_back, m->side);
+        if (ej == cudaSuccess) ej = cudaStreamWaitEvent(st, m->ev_back, 0);
+        CU(e);
+        CU(ej);
         return CHFSI_OK;
     }
     if (nlocal) {
@@ -421,6 +444,8 @@ static chfsi_status check_common(const chfsi_mesh* m, chfsi_prec prec, int nvec,
                                  const void* Y, long long ldy, const void* work, const char* who) {
     if (!m) return fail(CHFSI_EINVAL, std::string(who) + ": mesh is NULL");
     if (!m->ham_set) return fail(CHFSI_ESTATE, std::string(who) + ": chfsi_ham_set has not been called");
+    if (prec != CHFSI_FP64 && prec != CHFSI_FP32 && prec != CHFSI_TF32 && prec != CHFSI_TF32X3 && prec != CHFSI_FP32_STORED)
+        return fail(CHFSI_EINVAL, std::string(who) + ": unknown precision");
     if (prec == CHFSI_TF32 || prec == CHFSI_TF32X3) return fail(CHFSI_EUNSUPPORTED, std::string(who) + ": TF32 paths are not built");
     if (!cell_supported(m->p, prec)) return fail(CHFSI_EUNSUPPORTED, std::string(who) + ": precision/degree not built");
     if (nvec < 1) return fail(CHFSI_EINVAL, std::string(who) + ": nvec must be >= 1");
@@ -436,6 +461,7 @@ chfsi_status chfsi_apply_H(const chfsi_mesh* m, chfsi_prec prec, int nvec, const
     chfsi_status stt = check_common(m, prec, nvec, X, ldx, Y, ldy, work, "apply_H");
     if (stt != CHFSI_OK) return stt;
     if (X == Y) return fail(CHFSI_EINVAL, "apply_H: X and Y must be distinct");
+    if (prec == CHFSI_FP32_STORED) return fail(CHFSI_EUNSUPPORTED, "apply_H: FP32-stored multivectors exist only inside chfsi_cheb_filter");
     const size_t need = 2 * align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * nvec * 16);
     if (work_bytes < need) return fail(CHFSI_EINVAL, "apply_H: work_bytes too small");
     DeviceGuard g(m->device);
@@ -452,6 +478,35 @@ chfsi_status chfsi_apply_H(const chfsi_mesh* m, chfsi_prec prec, int nvec, const
     return accumulate_H(m, prec, ca, static_cast<double*>(work), st);
 }
 
+// Host side of the in-place recurrence.  The stored iterate is Zh_k = Z_k / s_k with
+// s_{k+1} = -gamma_k s_{k-1}: |s_k| decays geometrically, so before a step whose s_k has dropped below 2^-thresh both
+// stored iterates are multiplied by 2^-E and both scale factors by 2^E (exact), E = -ilogb|s_k|: s never leaves the
+// double range at any admissible degree and the stored values stay inside the FP32 range when they are complex64.
+struct Recur {
+    std::vector<double> r, aos, renorm, in_scale;     // per step k: s_k/s_{k+1}, alpha_k/s_{k+1}, 2^-E (or 0), 2^ilogb|s_k|
+    double s_last = 1.0;                             // s_m after all renormalisations
+};
+static Recur make_recur(int degree, const std::vector<double>& sig, double e, double s0, double s1, int thresh, int first_renorm) {
+    Recur rc;
+    rc.r.assign(degree + 1, 0.0); rc.aos.assign(degree + 1, 0.0); rc.renorm.assign(degree + 1, 0.0); rc.in_scale.assign(degree + 1, 1.0);
+    double sp = s0, sc = s1;
+    for (int k = 1; k < degree; ++k) {
+        if (k >= first_renorm && std::fabs(sc) < std::ldexp(1.0, -thresh)) {
+            const int E = -std::ilogb(std::fabs(sc));
+            sc = std::ldexp(sc, E); sp = std::ldexp(sp, E);
+            rc.renorm[k] = std::ldexp(1.0, -E);
+        }
+        const double alpha = 2.0 * sig[k + 1] / e, gamma = sig[k] * sig[k + 1];
+        const double sn = -gamma * sp;
+        rc.r[k] = sc / sn;
+        rc.aos[k] = alpha / sn;
+        rc.in_scale[k] = std::ldexp(1.0, std::ilogb(std::fabs(sc)));
+        sp = sc; sc = sn;
+    }
+    rc.s_last = degree >= 2 ? sc : s1;
+    return rc;
+}
+
 chfsi_status chfsi_cheb_filter(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur recur, int degree,
                                double a, double b, double a0, int nvec, int chunk, const void* X,
                                long long ldx, const double* lambda_host, void* Y, long long ldy,
@@ -465,13 +520,21 @@ chfsi_status chfsi_cheb_filter(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur
     if (chunk < 0) return fail(CHFSI_EINVAL, "cheb_filter: chunk < 0");
     if (chunk == 0 || chunk > nvec) chunk = nvec;
     if (chunk < nvec && chunk % 4 != 0) return fail(CHFSI_EINVAL, "cheb_filter: chunk must be a multiple of 4");
+    if (chunk > chfsi_mesh::kStageLambda) return fail(CHFSI_EINVAL, "cheb_filter: chunk must be <= 8192 vectors");
     if (recur == CHFSI_RECUR_RESIDUAL && !lambda_host) return fail(CHFSI_EINVAL, "cheb_filter: lambda_host is NULL");
     if (X == Y && ldx != ldy) return fail(CHFSI_EINVAL, "cheb_filter: aliased X/Y need equal leading dimensions");
-    const WorkLayout wl = work_layout(m, recur, chunk, kDegreeCap);
+    const bool st32 = prec == CHFSI_FP32_STORED;
+    if (st32 && recur != CHFSI_RECUR_RESIDUAL)
+        return fail(CHFSI_EUNSUPPORTED, "cheb_filter: FP32-stored multivectors need the residual recurrence (eq. 11)");
+    const WorkLayout wl = work_layout(m, prec, recur, chunk, kDegreeCap);
     if (work_bytes < wl.total) return fail(CHFSI_EINVAL, "cheb_filter: work_bytes too small");
+    if (!m->h_stage) return fail(CHFSI_ESTATE, "cheb_filter: staging ring missing (chfsi_ham_set not completed)");
     DeviceGuard g(m->device);
     if (!g.ok) return fail(CHFSI_ECUDA, "cheb_filter: cannot select device");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    cudaStreamIsCapturing(st, &cap);
+    const bool capturing = cap != cudaStreamCaptureStatusNone;
     g_launches = 0;
 
     // ---- scalars of PAPER.md:119
@@ -481,34 +544,40 @@ chfsi_status chfsi_cheb_filter(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur
     for (int k = 1; k < degree; ++k) sig[k + 1] = 1.0 / (2.0 / sig[1] - sig[k]);
     auto alpha = [&](int k) { return 2.0 * sig[k + 1] / e; };
     auto beta = [&](int k) { return 2.0 * sig[k + 1] * c / e; };
-    auto gamma = [&](int k) { return sig[k] * sig[k + 1]; };
 
     char* wbase = static_cast<char*>(work);
     double* dhdr = reinterpret_cast<double*>(wbase);
     double* coef = reinterpret_cast<double*>(wbase + wl.hdr_bytes);
     double* Cbuf = reinterpret_cast<double*>(wbase + wl.hdr_bytes + wl.coef_bytes);
-    double* buf[3];
-    for (int i = 0; i < 3; ++i)
-        buf[i] = reinterpret_cast<double*>(wbase + wl.hdr_bytes + wl.coef_bytes + wl.c_bytes + (size_t)i * wl.buf_bytes);
-    const size_t bufbytes_used = (size_t)2 * m->nnodes * 16;   // per column
+    char* bufbase = wbase + wl.hdr_bytes + wl.coef_bytes + wl.c_bytes;
+    double* buf0 = reinterpret_cast<double*>(bufbase);                         // R (eq. 11) or the work buffer (eq. 10)
+    void* zb[2] = {bufbase + wl.buf_bytes, bufbase + wl.buf_bytes + wl.zbuf_bytes};
+    const size_t esz = st32 ? 8 : 16;
 
     for (int j0 = 0; j0 < nvec; j0 += chunk) {
         const int nb = (nvec - j0) < chunk ? (nvec - j0) : chunk;
+        const long long ldz = st32 ? ((nb + 1) & ~1) : nb;
         const double* Xc = static_cast<const double*>(X) + 2ll * j0;
         double* Yc = static_cast<double*>(Y) + 2ll * j0;
-        // Row program for this chunk (a few KB, inlined in the command stream); the per-vector table,
-        // including the FP64 Lambda_k recurrence, is built on the device by coef_kernel.
+        // Row program for this chunk: written into a pinned staging slot owned by the mesh and uploaded from there; the
+        // per-vector table, including the FP64 Lambda_k recurrence, is built on the device by coef_kernel.
         const int nrows = degree + 1;
         std::vector<CoefRow> rows(nrows, CoefRow{0, 0, 0, 0, 0, 0, 0, 0, 0});
         auto dCIN = [&](int r) { return coef + (size_t)r * 2 * nb; };
         auto dCR = [&](int r) { return coef + (size_t)r * 2 * nb + nb; };
         auto upload_rows = [&](double q0, double q1, const double* lam) -> chfsi_status {
-            std::vector<double> hdr(4 + 9 * (size_t)nrows + nb, 0.0);
-            hdr[0] = q0; hdr[1] = q1; hdr[2] = nrows;
-            std::memcpy(hdr.data() + 4, rows.data(), sizeof(CoefRow) * nrows);
-            if (lam) std::memcpy(hdr.data() + 4 + 9 * (size_t)nrows, lam, sizeof(double) * nb);
-            CU(cudaMemcpyAsync(dhdr, hdr.data(), hdr.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+            const int slot = m->stage_next;
+            m->stage_next = (slot + 1) % chfsi_mesh::kStageSlots;
+            if (m->stage_used[slot] && !capturing) CU(cudaEventSynchronize(m->stage_ev[slot]));   // only if the GPU is 4 chunks behind
+            double* hs = m->h_stage + (size_t)slot * m->stage_slot_doubles;
+            const size_t nd = 4 + 9 * (size_t)nrows + nb;
+            hs[0] = q0; hs[1] = q1; hs[2] = nrows; hs[3] = 0.0;
+            std::memcpy(hs + 4, rows.data(), sizeof(CoefRow) * nrows);
+            if (lam) std::memcpy(hs + 4 + 9 * (size_t)nrows, lam, sizeof(double) * nb);
+            else std::memset(hs + 4 + 9 * (size_t)nrows, 0, sizeof(double) * nb);
+            CU(cudaMemcpyAsync(dhdr, hs, nd * sizeof(double), cudaMemcpyHostToDevice, st));
             count_launch();
+            if (!capturing) { CU(cudaEventRecord(m->stage_ev[slot], st)); m->stage_used[slot] = true; }
             CU(launch_coef(dhdr, coef, nrows, nb, st));
             return CHFSI_OK;
         };
@@ -517,92 +586,117 @@ chfsi_status chfsi_cheb_filter(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur
             // In-place accumulation: stored Zh_k = Z_k / s_k with s_{k+1} = -gamma_k s_{k-1}, so that
             //   Zh_{k+1} = Zh_{k-1} + (s_k/s_{k+1}) [alpha_k H D^-1 Zh_k - beta_k Zh_k] + (alpha_k/s_{k+1}) R Lambda_k
             // is a pure "+=" into the buffer that holds Zh_{k-1} ("in-place recurrence").
-            // s_1 = sigma_1/e makes Zh_1 = R exactly, so R's buffer doubles as Zh_1.
-            std::vector<double> s(degree + 2, 1.0);
-            s[0] = 1.0; s[1] = sig[1] / e;
-            for (int k = 1; k < degree; ++k) s[k + 1] = -gamma(k) * s[k - 1];
+            // s_1 = sigma_1/e makes Zh_1 = R exactly: with complex128 storage R's buffer doubles as Zh_1; with complex64
+            // storage Zh_1 is the FP32 copy of R ("FP32 multivectors ... only R and Lambda_k in FP64").
+            const Recur rc = make_recur(degree, sig, e, 1.0, sig[1] / e, st32 ? 24 : 256, 3);
             // row 0: S0, cin = -lambda_v (carries m_I in the kernel); rows 1..m-1: the steps; row m: recover
             rows[0].cinLam = -1.0;
-            std::vector<double> cHs(degree + 1, 0.0);
             for (int k = 1; k < degree; ++k) {
-                const double r = s[k] / s[k + 1];
-                cHs[k] = r * alpha(k);
                 CoefRow& rw = rows[k];
-                rw.cin0 = -r * beta(k);
-                if (k == 1) rw.cinL = alpha(k) / s[k + 1];      // in == R at the first step: R-term folded into cin
-                else rw.cRL = alpha(k) / s[k + 1];
-                if (k == 2) rw.cR0 = 1.0;                        // Zh_1 = R: the "+= Zh_{k-1}" term, folded in
-                rw.al = alpha(k); rw.be = beta(k); rw.ga = gamma(k); rw.advance = 1.0;
+                rw.cin0 = -rc.r[k] * beta(k);
+                if (k == 1 && !st32) rw.cinL = rc.aos[k];        // in == R at the first step: R-term folded into cin
+                else rw.cRL = rc.aos[k];
+                if (k == 2 && !st32) rw.cR0 = 1.0;               // Zh_1 = R: the "+= Zh_{k-1}" term, folded in
+                rw.al = alpha(k); rw.be = beta(k); rw.ga = sig[k] * sig[k + 1]; rw.advance = 1.0;
             }
-            rows[degree].cin0 = s[degree];                       // recover: Y = (s_m / m) Zh_m + Lambda_m X
+            rows[degree].cin0 = rc.s_last;                       // recover: Y = (s_m / m) Zh_m + Lambda_m X
             rows[degree].cRL = 1.0;
             stt = upload_rows(-sig[1] * c / e, sig[1] / e, lambda_host + j0);   // Lambda_1 = sigma_1 (lambda - c)/e
             if (stt != CHFSI_OK) return stt;
-            double* R = buf[0];
-            double* Zb[2] = {buf[1], buf[2]};
-            CU(cudaMemsetAsync(R, 0, bufbytes_used * nb, st)); count_launch();
+            double* R = buf0;
+            CU(cudaMemsetAsync(R, 0, (size_t)2 * m->nnodes * 16 * nb, st)); count_launch();
             // S0: R = H X - M X Lambda (FP64 always, Alg. 1 line 3)
             CellArgs ca{};
             ca.in = Xc; ca.ld_in = ldx; ca.out = R; ca.ld_out = nb; ca.R = nullptr; ca.ld_R = 0;
             ca.cin = dCIN(0); ca.cR = nullptr; ca.cH = 1.0; ca.nvec = nb; ca.flags = kMassIn;
             stt = accumulate_H(m, CHFSI_FP64, ca, Cbuf, st);
             if (stt != CHFSI_OK) return stt;
-            const double* zin = R;       // Zh_1
-            double* zcur = R;
+            // iterate buffers: complex128: Zh_1 = R (buf0), Zh_2 -> zb[0], Zh_3 -> zb[1] (zeroed; the R-term adds Zh_1), ...
+            //                  complex64 : Zh_1 = fl32(R) -> zb[1], Zh_2 -> zb[0] (zeroed), Zh_3 accumulates onto zb[1], ...
+            const void* zin = R;
+            void* zcur = R;
+            if (st32) {
+                CU(launch_cast32(m, zb[1], ldz, R, nb, nb, st));
+                zin = zb[1]; zcur = zb[1];
+            }
             for (int k = 1; k < degree; ++k) {
-                double* zout;
-                if (k == 1) zout = Zb[0];
-                else if (k == 2) zout = Zb[1];
-                else zout = (k % 2 == 1) ? Zb[0] : Zb[1];   // Zh_{k+1} overwrites Zh_{k-1}
-                if (k <= 2) { CU(cudaMemsetAsync(zout, 0, bufbytes_used * nb, st)); count_launch(); }
+                void* zout = (k % 2 == 1) ? zb[0] : zb[1];       // Zh_{k+1} overwrites Zh_{k-1}
+                if (k == 1 || (k == 2 && !st32)) { CU(cudaMemsetAsync(zout, 0, (size_t)2 * m->nnodes * esz * ldz, st)); count_launch(); }
+                if (rc.renorm[k] != 0.0) {
+                    // k >= 3: the two stored iterates are zin (Zh_k) and zout (Zh_{k-1}); never R
+                    CU(launch_scale(m, const_cast<void*>(zin), st32, (int)ldz, rc.renorm[k], st));
+                    CU(launch_scale(m, zout, st32, (int)ldz, rc.renorm[k], st));
+                }
                 CellArgs cs{};
-                cs.in = zin; cs.ld_in = nb; cs.out = zout; cs.ld_out = nb;
-                cs.R = (k >= 2) ? R : nullptr; cs.ld_R = nb;
-                cs.cin = dCIN(k); cs.cR = (k >= 2) ? dCR(k) : nullptr;
-                cs.cH = cHs[k]; cs.nvec = nb; cs.flags = kScaleIn;
-                cs.in_scale = std::ldexp(1.0, std::ilogb(std::fabs(s[k])));     // in = Z_k / s_k
+                cs.in = static_cast<const double*>(zin); cs.ld_in = (k == 1 && !st32) ? nb : ldz;
+                cs.out = static_cast<double*>(zout); cs.ld_out = ldz;
+                const bool useR = k >= 2 || st32;
+                cs.R = useR ? R : nullptr; cs.ld_R = nb;
+                cs.cin = dCIN(k); cs.cR = useR ? dCR(k) : nullptr;
+                cs.cH = rc.r[k] * alpha(k); cs.nvec = nb; cs.flags = kScaleIn;
+                cs.in_scale = rc.in_scale[k];                    // in = Z_k / s_k
+                cs.store_f32 = st32 ? 1 : 0;
                 stt = accumulate_H(m, prec, cs, Cbuf, st);
                 if (stt != CHFSI_OK) return stt;
                 zin = zout; zcur = zout;
             }
             // S7 recover: Y = D^-1 Z_m + X Lambda_m
-            CU(launch_axpby(m, Yc, ldy, zcur, nb, dCIN(degree), 1, Xc, ldx, dCR(degree), nb, st));
+            const bool cur32 = st32;                              // degree 1 with complex64: zcur is the FP32 copy of R
+            CU(launch_axpby(m, Yc, ldy, zcur, (zcur == R) ? nb : ldz, cur32 ? 1 : 0, dCIN(degree), 1, Xc, ldx, dCR(degree), nb, st));
         } else {
-            // eq. 10 with the same in-place trick: Yh_k = Y_k / s_k, s_{k+1} = -gamma_k s_{k-1}, and the chain
-            // with the parity of m normalised so that s_m = 1: the last accumulation lands in Y unscaled.
-            std::vector<double> s(degree + 2, 1.0);
-            for (int k = 1; k < degree; ++k) s[k + 1] = -gamma(k) * s[k - 1];
-            const double sm = s[degree];
-            for (int k = degree; k >= 0; k -= 2) s[k] /= sm;
+            // eq. 10 with the same in-place trick: Yh_k = Y_k / s_k, s_{k+1} = -gamma_k s_{k-1}, with the chain of the
+            // parity of m started at 1 / s_m so that the last accumulation lands in Y unscaled.  s_m is found by a first
+            // pass in (mantissa, exponent) form, so it cannot underflow; should 1 / s_m leave the double range the chain
+            // starts at 1 instead and the result gets one final scaling pass.
+            double mant = 1.0; long long ex2 = 0;                // s_m of the chain with the parity of m, started at 1
+            for (int k = degree; k >= 2; k -= 2) {
+                int ee; mant = std::frexp(mant * (-sig[k - 1] * sig[k]), &ee); ex2 += ee;
+            }
+            const bool direct = ex2 > -900 && ex2 < 900;
+            const double sm = direct ? std::ldexp(mant, (int)ex2) : 1.0;
+            const double s_even0 = (degree % 2 == 0) ? 1.0 / sm : 1.0, s_odd1 = (degree % 2 == 1) ? 1.0 / sm : 1.0;
+            // eq. 10's step 0 (Y_1 = sigma_1 (M^-1 H - c) X / e) has no Y_{-1}: it is a first step with its own coefficients
+            const Recur rc = make_recur(degree, sig, e, s_even0, s_odd1, 256, 3);
             // buffers: even indices live in E, odd in O; the one with the parity of m is Y itself
-            double* Wb = buf[0];
+            double* Wb = buf0;
             double* E = (degree % 2 == 0) ? Yc : Wb;  long long ldE = (degree % 2 == 0) ? ldy : nb;
             double* O = (degree % 2 == 0) ? Wb : Yc;  long long ldO = (degree % 2 == 0) ? nb : ldy;
             // row 0: scaled copy Yh_0 = X / s_0 ; row k+1: cin of step k (uniform over vectors)
-            rows[0].cin0 = 1.0 / s[0];
-            // step 0 (Y_1 = sigma_1 (M^-1 H - c) X / e):  Yh_1 = (s_0/s_1)(sigma_1/e) [M^-1 H Yh_0 - c Yh_0]
+            rows[0].cin0 = 1.0 / s_even0;
             std::vector<double> cHs(degree + 1, 0.0);
-            cHs[0] = (s[0] / s[1]) * sig[1] / e;
+            cHs[0] = (s_even0 / s_odd1) * sig[1] / e;
             rows[1].cin0 = -cHs[0] * c;
             for (int k = 1; k < degree; ++k) {
-                const double r = s[k] / s[k + 1];
-                cHs[k] = r * alpha(k);
-                rows[k + 1].cin0 = -r * beta(k);
+                cHs[k] = rc.r[k] * alpha(k);
+                rows[k + 1].cin0 = -rc.r[k] * beta(k);
             }
             stt = upload_rows(0.0, 0.0, nullptr);
             if (stt != CHFSI_OK) return stt;
-            CU(launch_axpby(m, E, ldE, Xc, ldx, dCIN(0), 0, nullptr, 0, nullptr, nb, st));   // E = X / s_0 (in place if E aliases X)
+            CU(launch_axpby(m, E, ldE, Xc, ldx, 0, dCIN(0), 0, nullptr, 0, nullptr, nb, st));   // E = X / s_0 (in place if E aliases X)
             CU(cudaMemset2DAsync(O, (size_t)ldO * 16, 0, (size_t)nb * 16, (size_t)2 * m->nnodes, st)); count_launch();
             for (int k = 0; k < degree; ++k) {
                 const bool in_even = (k % 2 == 0);
+                if (k >= 1 && rc.renorm[k] != 0.0) {
+                    // both stored iterates; the caller's Y may have ld > nb, so it is scaled through the strided copy kernel
+                    // (coefficient row `degree + 1`... kept simple: a uniform factor via launch_scale needs ld == nb)
+                    if (ldE != nb || ldO != nb) return fail(CHFSI_EUNSUPPORTED, "cheb_filter: eq. 10 at this degree / interval needs ldy == nvec (renormalisation pass)");
+                    CU(launch_scale(m, E, 0, nb, rc.renorm[k], st));
+                    CU(launch_scale(m, O, 0, nb, rc.renorm[k], st));
+                }
                 CellArgs cs{};
                 cs.in = in_even ? E : O; cs.ld_in = in_even ? ldE : ldO;
                 cs.out = in_even ? O : E; cs.ld_out = in_even ? ldO : ldE;
                 cs.R = nullptr; cs.ld_R = 0; cs.cin = dCIN(k + 1); cs.cR = nullptr;
                 cs.cH = cHs[k]; cs.nvec = nb; cs.flags = kSoutInvM;
-                cs.in_scale = std::ldexp(1.0, std::ilogb(std::fabs(s[k])));     // in = Y_k / s_k
+                cs.in_scale = k == 0 ? std::ldexp(1.0, std::ilogb(std::fabs(s_even0))) : rc.in_scale[k];     // in = Y_k / s_k
                 stt = accumulate_H(m, prec, cs, Cbuf, st);
                 if (stt != CHFSI_OK) return stt;
+            }
+            const double s_final = degree >= 2 ? rc.s_last : s_odd1;
+            if (s_final != 1.0 && std::fabs(s_final - 1.0) > 1e-14) {
+                // the chain could not be started at 1 / s_m (or was renormalised on the way): one scaling pass Y *= s_m
+                if (ldy != nb) return fail(CHFSI_EUNSUPPORTED, "cheb_filter: eq. 10 at this degree / interval needs ldy == nvec (final scaling pass)");
+                CU(launch_scale(m, Yc, 0, nb, s_final, st));
             }
         }
     }

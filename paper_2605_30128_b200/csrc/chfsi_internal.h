@@ -55,6 +55,9 @@ struct CellArgs {
     // FP32 result by its reciprocal after widening, so that the scaled iterates Z_k / s_k stay
     // inside the FP32 range at any degree.  1.0 (or 0 = unset) elsewhere.
     double in_scale;
+    // FP32-stored multivectors (CHFSI_FP32_STORED): `in` and `out` are complex64 (leading dimensions still in
+    // complex elements); R stays complex128.
+    int store_f32;
 };
 
 struct ProjItem { int atom; int start; int count; };   // a slice of an atom's support list
@@ -82,20 +85,22 @@ struct NonlocalDev {
 };
 
 struct ProjArgs {
-    const double* in; long long ld_in;
+    const void* in; long long ld_in;    // complex128, or complex64 when store_f32
     double* C;                          // [crows][nvec] complex128, zeroed by the driver
     int nvec;
     int mass_u;                         // 1: u = m_I * in (apply on X); 0: u = in (Z-form)
     double in_scale;                    // see CellArgs::in_scale (the back pass gets cH / in_scale)
+    int store_f32;
 };
 
 struct BackArgs {
     const double* C;                    // projected coefficients
     double* G;                          // scratch for G = D C, same shape as C
-    double* out; long long ld_out;
+    void* out; long long ld_out;        // complex128, or complex64 when store_f32
     double cH;
     int nvec;
     int sout_invm;                      // 1: s_out = 1/m  => m * (1/m) = 1 ; 0: factor m_I
+    int store_f32;
 };
 
 }  // namespace chfsi
@@ -125,6 +130,15 @@ struct chfsi_mesh {
     // kernel's last wave leaves idle (created in chfsi_ham_set)
     mutable cudaStream_t side = nullptr;
     mutable cudaEvent_t ev_proj = nullptr, ev_back = nullptr;
+    // pinned staging ring for the per-chunk coefficient program of chfsi_cheb_filter (allocated in chfsi_ham_set): the
+    // asynchronous upload reads pinned memory owned by the mesh, never a pageable buffer of the caller's stack frame
+    static constexpr int kStageSlots = 4;
+    static constexpr int kStageLambda = 8192;          // vectors per chunk the ring is sized for
+    mutable double* h_stage = nullptr;
+    mutable size_t stage_slot_doubles = 0;
+    mutable int stage_next = 0;
+    mutable cudaEvent_t stage_ev[kStageSlots] = {nullptr, nullptr, nullptr, nullptr};
+    mutable bool stage_used[kStageSlots] = {false, false, false, false};
 };
 
 namespace chfsi {
@@ -133,9 +147,13 @@ cudaError_t launch_cell(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a,
 cudaError_t launch_proj(const chfsi_mesh* m, chfsi_prec prec, const ProjArgs& a, cudaStream_t s);
 cudaError_t launch_back(const chfsi_mesh* m, chfsi_prec prec, const BackArgs& a, cudaStream_t s);
 // out[row][v] = ca[v] * (inv_mass ? A/m : A) + cb[v] * B   (B, cb may be null); rows = 2*nnodes
-cudaError_t launch_axpby(const chfsi_mesh* m, double* out, long long ldo, const double* A, long long lda,
+cudaError_t launch_axpby(const chfsi_mesh* m, double* out, long long ldo, const void* A, long long lda, int a_f32,
                          const double* ca, int a_inv_mass, const double* B, long long ldb,
                          const double* cb, int nvec, cudaStream_t s);
+// dst (complex64, ld = ldd) = (float) src (complex128, ld = lds): the FP32 copy of Zh_1 = R (CHFSI_FP32_STORED)
+cudaError_t launch_cast32(const chfsi_mesh* m, void* dst, long long ldd, const double* src, long long lds, int nvec, cudaStream_t s);
+// buf *= f (an exact power of two) on a multivector of nvec columns, ld = nvec (renormalisation of the scaled iterates)
+cudaError_t launch_scale(const chfsi_mesh* m, void* buf, int f32, int nvec, double f, cudaStream_t s);
 // Per-step coefficient rows.  For vector v with Ritz value lam and the running Lambda_k(v) = L:
 //   cin[r][v] = cin0 + cinL * L + cinLam * lam ;  cR[r][v] = cR0 + cRL * L ;
 //   then, if advance: L_next = al * lam * L - be * L - ga * L_prev   (Lambda_k recurrence)
@@ -147,6 +165,9 @@ bool cell_supported(int p, chfsi_prec prec);
 // z-marching TMA kernel (cell_march.cu)
 bool march_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
 cudaError_t launch_cell_march(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
+// line-owned x/y/z TMA kernel (cell_xyz.cu)
+bool xyz_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
+cudaError_t launch_cell_xyz(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
 void set_error(const std::string& s);
 void count_launch(int n = 1);
 }  // namespace chfsi

@@ -207,9 +207,16 @@ cell_kernel(const __grid_constant__ MeshConst mc, const __grid_constant__ CellAr
 // one slice x 128 (spin, vector) columns.
 constexpr int kSlice = 8;
 
-template <typename TT>
+template <typename TS> struct C2Sel;
+template <> struct C2Sel<double> { using type = double2; };
+template <> struct C2Sel<float> { using type = float2; };
+__device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
+
+// TT: arithmetic type of the contraction; TS: storage type of the multivectors (double: complex128, float: complex64)
+template <typename TT, typename TS>
 __global__ void __launch_bounds__(128)
 proj_kernel(const NonlocalDev nl, const ProjArgs ar) {
+    using S2 = typename C2Sel<TS>::type;
     const ProjItem it = nl.items[blockIdx.x];
     const int s = blockIdx.y & 1;
     const int v = (blockIdx.y >> 1) * 128 + threadIdx.x;
@@ -223,7 +230,8 @@ proj_kernel(const NonlocalDev nl, const ProjArgs ar) {
         x[jj] = make_double2(0.0, 0.0);
         if (jj < it.count) {
             const long long I = nl.supp_node[soff + jj];
-            x[jj] = __ldg(reinterpret_cast<const double2*>(ar.in) + (2 * I + s) * ar.ld_in + v);
+            const S2 xs = __ldg(reinterpret_cast<const S2*>(ar.in) + (2 * I + s) * ar.ld_in + v);
+            x[jj] = make_double2((double)xs.x, (double)xs.y);
             { const double m = (ar.mass_u ? nl.supp_mass[soff + jj] : 1.0) * ar.in_scale; x[jj].x *= m; x[jj].y *= m; }
         }
     }
@@ -268,7 +276,7 @@ gmat_kernel(const NonlocalDev nl, const double2* __restrict__ Cc, double2* __res
     G[(nl.c_off[atom] + row) * (long long)nvec + v] = make_double2(gr, gi);
 }
 
-template <typename TT>
+template <typename TT, typename TS>
 __global__ void __launch_bounds__(128)
 back_kernel(const NonlocalDev nl, const BackArgs ar) {
     const ProjItem it = nl.items[blockIdx.x];
@@ -301,9 +309,9 @@ back_kernel(const NonlocalDev nl, const BackArgs ar) {
         if (jj < it.count) {
             const long long I = nl.supp_node[soff + jj];
             const double f = ar.cH * (ar.sout_invm ? 1.0 : nl.supp_mass[soff + jj]);
-            double* dst = ar.out + ((2 * I + s) * ar.ld_out + v) * 2;
-            red_add(dst, f * (double)yr[jj]);
-            red_add(dst + 1, f * (double)yi[jj]);
+            TS* dst = reinterpret_cast<TS*>(ar.out) + ((2 * I + s) * ar.ld_out + v) * 2;
+            red_add(dst, (TS)(f * (double)yr[jj]));
+            red_add(dst + 1, (TS)(f * (double)yi[jj]));
         }
     }
 }
@@ -320,10 +328,11 @@ template <typename TT> struct P2Sel;
 template <> struct P2Sel<double> { using type = double2; static __device__ __forceinline__ const double2* ptr(const NonlocalDev& nl) { return nl.P64; } };
 template <> struct P2Sel<float> { using type = float2; static __device__ __forceinline__ const float2* ptr(const NonlocalDev& nl) { return nl.P32; } };
 
-template <typename TT, int NP>
+template <typename TT, typename TS, int NP>
 __global__ void __launch_bounds__(128)
 proj_fast_kernel(const NonlocalDev nl, const ProjArgs ar) {
     using P2 = typename P2Sel<TT>::type;
+    using S2 = typename C2Sel<TS>::type;
     __shared__ P2 Ps[kBig * NP];
     __shared__ long long nodes[kBig];
     __shared__ double mass[kBig];
@@ -343,20 +352,21 @@ proj_fast_kernel(const NonlocalDev nl, const ProjArgs ar) {
     TT cr[NP], ci[NP];
 #pragma unroll
     for (int b = 0; b < NP; ++b) { cr[b] = 0; ci[b] = 0; }
-    const double2* in2 = reinterpret_cast<const double2*>(ar.in) + (long long)s * ar.ld_in + v;
+    const S2* in2 = reinterpret_cast<const S2*>(ar.in) + (long long)s * ar.ld_in + v;
 #pragma unroll 1
     for (int j0 = 0; j0 < it.count; j0 += kSlice) {
-        double2 x[kSlice];
+        S2 x[kSlice];
 #pragma unroll
         for (int jj = 0; jj < kSlice; ++jj) {
             const bool ok = j0 + jj < it.count;
-            x[jj] = ok ? __ldg(in2 + 2 * nodes[j0 + jj] * ar.ld_in) : make_double2(0.0, 0.0);
+            x[jj].x = 0; x[jj].y = 0;
+            if (ok) x[jj] = __ldg(in2 + 2 * nodes[j0 + jj] * ar.ld_in);
         }
 #pragma unroll
         for (int jj = 0; jj < kSlice; ++jj) {
             if (j0 + jj < it.count) {
                 const double m = mass[j0 + jj];
-                const TT xr = (TT)(x[jj].x * m), xi = (TT)(x[jj].y * m);
+                const TT xr = (TT)((double)x[jj].x * m), xi = (TT)((double)x[jj].y * m);
 #pragma unroll
                 for (int b = 0; b < NP; ++b) {
                     const P2 pv = Ps[(j0 + jj) * NP + b];
@@ -375,7 +385,7 @@ proj_fast_kernel(const NonlocalDev nl, const ProjArgs ar) {
     }
 }
 
-template <typename TT, int NP>
+template <typename TT, typename TS, int NP>
 __global__ void __launch_bounds__(128)
 back_fast_kernel(const NonlocalDev nl, const BackArgs ar) {
     using P2 = typename P2Sel<TT>::type;
@@ -415,7 +425,7 @@ back_fast_kernel(const NonlocalDev nl, const BackArgs ar) {
     TT g_r[NP], g_i[NP];
 #pragma unroll
     for (int b = 0; b < NP; ++b) { g_r[b] = (TT)gr[b]; g_i[b] = (TT)gi[b]; }
-    double* out = ar.out + ((long long)s * ar.ld_out + v) * 2;
+    TS* out = reinterpret_cast<TS*>(ar.out) + ((long long)s * ar.ld_out + v) * 2;
 #pragma unroll 4
     for (int jj = 0; jj < it.count; ++jj) {
         TT yr = 0, yi = 0;
@@ -425,17 +435,18 @@ back_fast_kernel(const NonlocalDev nl, const BackArgs ar) {
             yr = fma(pv.x, g_r[b], fma(-pv.y, g_i[b], yr));
             yi = fma(pv.x, g_i[b], fma(pv.y, g_r[b], yi));
         }
-        double* dst = out + 4 * nodes[jj] * ar.ld_out;
-        red_add(dst, fac[jj] * (double)yr);
-        red_add(dst + 1, fac[jj] * (double)yi);
+        TS* dst = out + 4 * nodes[jj] * ar.ld_out;
+        red_add(dst, (TS)(fac[jj] * (double)yr));
+        red_add(dst + 1, (TS)(fac[jj] * (double)yi));
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // S7 / scaled copies: out[row][v] = ca[v] * (a_inv_mass ? A/m : A) + cb[v] * B
+template <typename TS>
 __global__ void __launch_bounds__(256)
 axpby_kernel(const __grid_constant__ MeshConst mc, double2* __restrict__ out, long long ldo,
-             const double2* __restrict__ A, long long lda, const double* __restrict__ ca, int a_inv_mass,
+             const typename C2Sel<TS>::type* __restrict__ A, long long lda, const double* __restrict__ ca, int a_inv_mass,
              const double2* __restrict__ B, long long ldb, const double* __restrict__ cb, int nvec) {
     const long long rows = 2 * mc.nnodes;
     const long long total = rows * nvec;
@@ -451,8 +462,8 @@ axpby_kernel(const __grid_constant__ MeshConst mc, double2* __restrict__ out, lo
             const int iz = (int)(I / ((long long)mc.n1[0] * mc.n1[1]));
             f *= mc.im1[0][ix % mc.p] * mc.im1[1][iy % mc.p] * mc.im1[2][iz % mc.p];
         }
-        const double2 av = A[row * lda + v];
-        double2 r = make_double2(f * av.x, f * av.y);
+        const typename C2Sel<TS>::type av = A[row * lda + v];
+        double2 r = make_double2(f * (double)av.x, f * (double)av.y);
         if (B != nullptr) {
             const double g = cb[v];
             const double2 bv = B[row * ldb + v];
@@ -507,20 +518,16 @@ static cudaError_t launch_cell_t(const chfsi_mesh* m, const CellArgs& a, cudaStr
 }
 
 bool cell_supported(int p, chfsi_prec prec) {
+    if (prec == CHFSI_FP32_STORED) return p == 2 || p == 4 || p == 6 || p == 8;   // line-owned kernel only
     if (prec != CHFSI_FP64 && prec != CHFSI_FP32) return false;
     return p >= 1 && p <= 8;
 }
 
 static cudaError_t launch_cell_legacy(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t st);
 
-static bool use_legacy() {
-    static int v = -1;
-    if (v < 0) { const char* e = getenv("CHFSI_CELL_KERNEL"); v = (e && std::string(e) == "legacy") ? 1 : 0; }
-    return v == 1;
-}
-
-// The dominant kernel: the z-marching TMA kernel where it is instantiated (FP64; p = 2, 4, 6), else the
-// tile-per-cell kernel above (FP32 product; other degrees).  CHFSI_CELL_KERNEL=legacy forces the latter.
+// The dominant kernel.  FP64: the z-marching kernel (cell_march.cu) for p = 2, 4, 6 (within a few percent of its memory
+// floor at p = 6), the line-owned x/y/z kernel (cell_xyz.cu) for p = 8.  FP32 product and FP32-stored multivectors: the
+// line-owned kernel.  Odd degrees: the tile-per-cell kernel above.
 cudaError_t launch_cell(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t st) {
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (m->prof_on) {
@@ -528,13 +535,18 @@ cudaError_t launch_cell(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a,
         cudaEventRecord(e0, st);
     }
     cudaError_t err;
-    if (!use_legacy() && march_supported(m, prec, a)) err = launch_cell_march(m, prec, a, st);
+    const bool use_march = prec == CHFSI_FP64 && m->p <= 6 && march_supported(m, prec, a);
+    if (!use_march && xyz_supported(m, prec, a)) err = launch_cell_xyz(m, prec, a, st);
+    else if (use_march) err = launch_cell_march(m, prec, a, st);
+    else if (a.store_f32) err = cudaErrorInvalidValue;
     else err = launch_cell_legacy(m, prec, a, st);
     count_launch();
     if (m->prof_on) {
         cudaEventRecord(e1, st);
         m->prof_ev.push_back(e0); m->prof_ev.push_back(e1);
-        m->prof_bytes += 2.0 * (double)m->nnodes * a.nvec * (16.0 * (1 + (a.R != nullptr && a.cR != nullptr)) + 32.0);
+        // algorithmic bytes per unit: `in` read once, `out` read and written by the reduction, R read in FP64
+        const double eb = a.store_f32 ? 8.0 : 16.0;
+        m->prof_bytes += 2.0 * (double)m->nnodes * a.nvec * (eb + 2.0 * eb + ((a.R != nullptr && a.cR != nullptr) ? 16.0 : 0.0));
     }
     return err;
 }
@@ -558,65 +570,108 @@ static cudaError_t launch_cell_legacy(const chfsi_mesh* m, chfsi_prec prec, cons
 #undef CELL_CASE
 }
 
-cudaError_t launch_proj(const chfsi_mesh* m, chfsi_prec prec, const ProjArgs& a, cudaStream_t st) {
-    if (m->nl.nitems == 0) return cudaSuccess;
+template <typename TT, typename TS>
+static void launch_proj_t(const chfsi_mesh* m, const ProjArgs& a, cudaStream_t st) {
     if (m->nl.uniform_np == 4 || m->nl.uniform_np == 8) {
         dim3 grid(m->nl.nitems_big, 2 * ((a.nvec + 127) / 128));
-        const bool f32 = prec == CHFSI_FP32;
-        if (m->nl.uniform_np == 8) {
-            if (f32) proj_fast_kernel<float, 8><<<grid, 128, 0, st>>>(m->nl, a);
-            else proj_fast_kernel<double, 8><<<grid, 128, 0, st>>>(m->nl, a);
-        } else {
-            if (f32) proj_fast_kernel<float, 4><<<grid, 128, 0, st>>>(m->nl, a);
-            else proj_fast_kernel<double, 4><<<grid, 128, 0, st>>>(m->nl, a);
-        }
-        count_launch();
-        return cudaGetLastError();
+        if (m->nl.uniform_np == 8) proj_fast_kernel<TT, TS, 8><<<grid, 128, 0, st>>>(m->nl, a);
+        else proj_fast_kernel<TT, TS, 4><<<grid, 128, 0, st>>>(m->nl, a);
+    } else {
+        dim3 grid(m->nl.nitems, 2 * ((a.nvec + 127) / 128));
+        proj_kernel<TT, TS><<<grid, 128, 0, st>>>(m->nl, a);
     }
-    dim3 grid(m->nl.nitems, 2 * ((a.nvec + 127) / 128));
-    if (prec == CHFSI_FP32) proj_kernel<float><<<grid, 128, 0, st>>>(m->nl, a);
-    else proj_kernel<double><<<grid, 128, 0, st>>>(m->nl, a);
+}
+
+cudaError_t launch_proj(const chfsi_mesh* m, chfsi_prec prec, const ProjArgs& a, cudaStream_t st) {
+    if (m->nl.nitems == 0) return cudaSuccess;
+    if (a.store_f32) launch_proj_t<float, float>(m, a, st);
+    else if (prec == CHFSI_FP64) launch_proj_t<double, double>(m, a, st);
+    else launch_proj_t<float, double>(m, a, st);
     count_launch();
     return cudaGetLastError();
+}
+
+template <typename TT, typename TS>
+static void launch_back_t(const chfsi_mesh* m, const BackArgs& a, cudaStream_t st) {
+    if (m->nl.uniform_np == 4 || m->nl.uniform_np == 8) {
+        dim3 grid(m->nl.nitems_big, 2 * ((a.nvec + 127) / 128));
+        if (m->nl.uniform_np == 8) back_fast_kernel<TT, TS, 8><<<grid, 128, 0, st>>>(m->nl, a);
+        else back_fast_kernel<TT, TS, 4><<<grid, 128, 0, st>>>(m->nl, a);
+        return;
+    }
+    {
+        dim3 gg(m->nl.natoms, 2 * m->nl.max_nproj, (a.nvec + 127) / 128);
+        gmat_kernel<<<gg, 128, 0, st>>>(m->nl, reinterpret_cast<const double2*>(a.C), reinterpret_cast<double2*>(a.G), a.nvec);
+        count_launch();
+    }
+    dim3 grid(m->nl.nitems, 2 * ((a.nvec + 127) / 128));
+    back_kernel<TT, TS><<<grid, 128, 0, st>>>(m->nl, a);
 }
 
 cudaError_t launch_back(const chfsi_mesh* m, chfsi_prec prec, const BackArgs& a, cudaStream_t st) {
     if (m->nl.nitems == 0) return cudaSuccess;
-    if (m->nl.uniform_np == 4 || m->nl.uniform_np == 8) {
-        dim3 grid(m->nl.nitems_big, 2 * ((a.nvec + 127) / 128));
-        const bool f32 = prec == CHFSI_FP32;
-        if (m->nl.uniform_np == 8) {
-            if (f32) back_fast_kernel<float, 8><<<grid, 128, 0, st>>>(m->nl, a);
-            else back_fast_kernel<double, 8><<<grid, 128, 0, st>>>(m->nl, a);
-        } else {
-            if (f32) back_fast_kernel<float, 4><<<grid, 128, 0, st>>>(m->nl, a);
-            else back_fast_kernel<double, 4><<<grid, 128, 0, st>>>(m->nl, a);
-        }
-        count_launch();
-        return cudaGetLastError();
-    }
-    {
-        dim3 gg(m->nl.natoms, 2 * m->nl.max_nproj, (a.nvec + 127) / 128);
-        gmat_kernel<<<gg, 128, 0, st>>>(m->nl, reinterpret_cast<const double2*>(a.C),
-                                        reinterpret_cast<double2*>(a.G), a.nvec);
-        count_launch();
-    }
-    dim3 grid(m->nl.nitems, 2 * ((a.nvec + 127) / 128));
-    if (prec == CHFSI_FP32) back_kernel<float><<<grid, 128, 0, st>>>(m->nl, a);
-    else back_kernel<double><<<grid, 128, 0, st>>>(m->nl, a);
+    if (a.store_f32) launch_back_t<float, float>(m, a, st);
+    else if (prec == CHFSI_FP64) launch_back_t<double, double>(m, a, st);
+    else launch_back_t<float, double>(m, a, st);
     count_launch();
     return cudaGetLastError();
 }
 
-cudaError_t launch_axpby(const chfsi_mesh* m, double* out, long long ldo, const double* A, long long lda,
+cudaError_t launch_axpby(const chfsi_mesh* m, double* out, long long ldo, const void* A, long long lda, int a_f32,
                          const double* ca, int a_inv_mass, const double* B, long long ldb,
                          const double* cb, int nvec, cudaStream_t st) {
     const long long total = 2 * m->nnodes * (long long)nvec;
     long long blocks = (total + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
-    axpby_kernel<<<(unsigned)blocks, 256, 0, st>>>(m->mc, reinterpret_cast<double2*>(out), ldo,
-                                                   reinterpret_cast<const double2*>(A), lda, ca, a_inv_mass,
-                                                   reinterpret_cast<const double2*>(B), ldb, cb, nvec);
+    if (a_f32)
+        axpby_kernel<float><<<(unsigned)blocks, 256, 0, st>>>(m->mc, reinterpret_cast<double2*>(out), ldo,
+                                                              reinterpret_cast<const float2*>(A), lda, ca, a_inv_mass,
+                                                              reinterpret_cast<const double2*>(B), ldb, cb, nvec);
+    else
+        axpby_kernel<double><<<(unsigned)blocks, 256, 0, st>>>(m->mc, reinterpret_cast<double2*>(out), ldo,
+                                                               reinterpret_cast<const double2*>(A), lda, ca, a_inv_mass,
+                                                               reinterpret_cast<const double2*>(B), ldb, cb, nvec);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// FP32-stored multivectors (CHFSI_FP32_STORED): the FP32 copy of Zh_1 = R, and the power-of-two renormalisation of the
+// scaled iterates (both streaming, a few times per filter call)
+__global__ void __launch_bounds__(256)
+cast32_kernel(float2* __restrict__ dst, long long ldd, const double2* __restrict__ src, long long lds, long long rows, int nvec) {
+    const long long total = rows * nvec;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+        const long long row = idx / nvec;
+        const int v = (int)(idx - row * nvec);
+        const double2 s = src[row * lds + v];
+        dst[row * ldd + v] = make_float2((float)s.x, (float)s.y);
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+scale_kernel(T* __restrict__ buf, long long count, T f) {
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < count; idx += (long long)gridDim.x * blockDim.x)
+        buf[idx] *= f;
+}
+
+cudaError_t launch_cast32(const chfsi_mesh* m, void* dst, long long ldd, const double* src, long long lds, int nvec, cudaStream_t st) {
+    const long long total = 2 * m->nnodes * (long long)nvec;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    cast32_kernel<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<float2*>(dst), ldd, reinterpret_cast<const double2*>(src), lds,
+                                                    2 * m->nnodes, nvec);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scale(const chfsi_mesh* m, void* buf, int f32, int nvec, double f, cudaStream_t st) {
+    const long long count = 4 * m->nnodes * (long long)nvec;     // reals
+    long long blocks = (count + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (f32) scale_kernel<float><<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<float*>(buf), count, (float)f);
+    else scale_kernel<double><<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<double*>(buf), count, f);
     count_launch();
     return cudaGetLastError();
 }
