@@ -158,6 +158,30 @@ chfsi_status chfsi_profile_enable(chfsi_mesh* mesh, int on);
 chfsi_status chfsi_profile_read(chfsi_mesh* mesh, double* cell_ms, long long* cell_launches,
                                 double* cell_alg_bytes);
 
+/* ---- block floating-point codec of the compressed ghost exchange (Fig. 3) -----------------
+ * Four FP32 values <-> one N_bits = 4 n_bits bit word, n_bits in {16, 12, 10}: bits 0..7 = shared biased exponent
+ * e = e_max + 127 with 2^(e_max-1) <= max|x_i| < 2^e_max (0 flags an all-zero block; FP32-subnormal maxima use
+ * e_max = -126), then four v_bits = n_bits - 2 bit two's-complement coefficients q_i = round(x_i 2^(v_bits-1-e_max))
+ * (ties to even, clamped above at 2^(v_bits-1) - 1), q_0 lowest; decode x~_i = q_i 2^(e_max-v_bits+1), exact.
+ * Stream layout: block b at byte offset b * n_bits / 2, little-endian ("a single uint64_t", "three uint16_t", "five
+ * uint8_t"), no padding.  Inputs must be finite.  One thread per block; no atomics in
+ * encode.  All pointers are device memory; work is enqueued on cuda_stream; nothing is allocated or synchronised.
+ * EINVAL: n_bits not in {16,12,10}, n < 0 or n % 4 != 0, NULL pointers with n > 0, misaligned pointers (FP32 / multi-
+ * vector side 16 B, stream side 8 B), nvec odd or ld odd or ld < nvec in the fused forms. */
+chfsi_status chfsi_bfp_stream_bytes(int nbits, long long n, size_t* bytes);      /* n n_bits / 8 */
+chfsi_status chfsi_bfp_encode(int nbits, const void* src_f32, long long n, void* dst_stream, void* cuda_stream);
+chfsi_status chfsi_bfp_decode(int nbits, const void* src_stream, long long n, void* dst_f32, void* cuda_stream);
+/* Fused forms.  rows: device, nrows (node, spin) row indices 2 I + alpha of the message, in order.
+ * The message is the FP32 values (re, im interleaved, vectors fastest) of those rows, 2 nvec values per row.
+ * gather_encode ("gathers the entries for each neighbour and encodes them in the same pass"): X is a complex128
+ * (complex_bytes 16; rounded to FP32 first) or complex64 (complex_bytes 8) multivector with leading dimension ld.
+ * decode_scatter_add ("decodes the data and atomically scatter-adds it to the corresponding owned entries"):
+ * Y[row] += decoded values, by atomic adds in Y's precision; a row may be listed several times. */
+chfsi_status chfsi_bfp_gather_encode(int nbits, const void* X, int complex_bytes, long long ld, int nvec,
+                                     const long long* rows, long long nrows, void* dst_stream, void* cuda_stream);
+chfsi_status chfsi_bfp_decode_scatter_add(int nbits, const void* src_stream, const long long* rows, long long nrows,
+                                          int nvec, void* Y, int complex_bytes, long long ld, void* cuda_stream);
+
 const char* chfsi_last_error(void);     /* thread-local; never NULL */
 const char* chfsi_version(void);
 

@@ -24,6 +24,8 @@ EXPORTS = [
     "chfsi_mesh_create", "chfsi_mesh_destroy", "chfsi_mesh_num_nodes", "chfsi_mesh_node_coords",
     "chfsi_mesh_mass", "chfsi_ham_set", "chfsi_workspace_bytes", "chfsi_apply_H", "chfsi_cheb_filter",
     "chfsi_profile_enable", "chfsi_profile_read",
+    "chfsi_bfp_stream_bytes", "chfsi_bfp_encode", "chfsi_bfp_decode", "chfsi_bfp_gather_encode",
+    "chfsi_bfp_decode_scatter_add",
     "chfsi_last_launch_count", "chfsi_last_error", "chfsi_version",
 ]
 
@@ -59,8 +61,14 @@ def lib() -> C.CDLL:
                                     C.c_size_t, vp]
     L.chfsi_profile_enable.argtypes = [vp, C.c_int]
     L.chfsi_profile_read.argtypes = [vp, dp, llp, dp]
-    for name in EXPORTS[:11]:
-        getattr(L, name).restype = C.c_int
+    L.chfsi_bfp_stream_bytes.argtypes = [C.c_int, C.c_longlong, C.POINTER(C.c_size_t)]
+    L.chfsi_bfp_encode.argtypes = [C.c_int, vp, C.c_longlong, vp, vp]
+    L.chfsi_bfp_decode.argtypes = [C.c_int, vp, C.c_longlong, vp, vp]
+    L.chfsi_bfp_gather_encode.argtypes = [C.c_int, vp, C.c_int, C.c_longlong, C.c_int, vp, C.c_longlong, vp, vp]
+    L.chfsi_bfp_decode_scatter_add.argtypes = [C.c_int, vp, vp, C.c_longlong, C.c_int, vp, C.c_int, C.c_longlong, vp]
+    for name in EXPORTS:
+        if name not in ("chfsi_last_launch_count", "chfsi_last_error", "chfsi_version"):
+            getattr(L, name).restype = C.c_int
     L.chfsi_last_launch_count.restype = C.c_longlong
     L.chfsi_last_error.restype = C.c_char_p
     L.chfsi_version.restype = C.c_char_p
@@ -189,3 +197,30 @@ def chfsi_last_launch_count() -> int:
 
 def chfsi_version() -> str:
     return lib().chfsi_version().decode()
+
+
+# ---- BFP codec ----------------------------------------------------------------
+def chfsi_bfp_stream_bytes(nbits, n) -> int:
+    b = C.c_size_t()
+    _check(lib().chfsi_bfp_stream_bytes(int(nbits), int(n), C.byref(b)))
+    return b.value
+
+
+def chfsi_bfp_encode(nbits, src, dst, stream=None):
+    """src: torch float32 CUDA tensor (numel % 4 == 0); dst: torch uint8 CUDA tensor of chfsi_bfp_stream_bytes."""
+    _check(lib().chfsi_bfp_encode(int(nbits), _ptr(src), src.numel(), _ptr(dst), _stream(stream)))
+
+
+def chfsi_bfp_decode(nbits, src, dst, stream=None):
+    _check(lib().chfsi_bfp_decode(int(nbits), _ptr(src), dst.numel(), _ptr(dst), _stream(stream)))
+
+
+def chfsi_bfp_gather_encode(nbits, X, rows, dst, stream=None):
+    """X: torch complex128 / complex64 CUDA tensor [nrows_total, ld]; rows: torch int64 CUDA tensor."""
+    _check(lib().chfsi_bfp_gather_encode(int(nbits), _ptr(X), X.element_size(), X.stride(0), X.shape[1], _ptr(rows),
+                                         rows.numel(), _ptr(dst), _stream(stream)))
+
+
+def chfsi_bfp_decode_scatter_add(nbits, src, rows, Y, stream=None):
+    _check(lib().chfsi_bfp_decode_scatter_add(int(nbits), _ptr(src), _ptr(rows), rows.numel(), Y.shape[1], _ptr(Y),
+                                              Y.element_size(), Y.stride(0), _stream(stream)))

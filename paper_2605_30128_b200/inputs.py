@@ -294,3 +294,17 @@ def lanczos_start(nnodes: int, seed: int = 0) -> np.ndarray:
     """Seeded start vector [nnodes,2,1] for the harness/oracle Lanczos bound estimate (A4)."""
     rng = np.random.default_rng([seed, 104])
     return (rng.standard_normal((nnodes, 2, 1)) + 1j * rng.standard_normal((nnodes, 2, 1)))
+
+
+def make_ghost_values(n: int, seed: int = 0, rows_of: int = 64) -> np.ndarray:
+    """Seeded FP32 stand-in for an exchanged face slab of residual iterates ("exchanged residual values
+    associated with neighbouring nodes typically have similar magnitudes and tend toward zero"): runs of `rows_of` values
+    share a log-uniform magnitude in 2^[-24, 4], individual values are Gaussian around it, 2 % exact zeros and a few whole
+    zero runs.  No codec arithmetic here."""
+    rng = np.random.default_rng([seed, 77])
+    nrun = (n + rows_of - 1) // rows_of
+    mag = np.exp2(rng.uniform(-24.0, 4.0, size=nrun))
+    mag[rng.random(nrun) < 0.02] = 0.0
+    x = rng.standard_normal((nrun, rows_of)) * mag[:, None]
+    x[rng.random((nrun, rows_of)) < 0.02] = 0.0
+    return x.astype(np.float32).ravel()[:n].copy()
