@@ -55,14 +55,25 @@ typedef enum {
 typedef enum {
     CHFSI_FP64 = 0,          /* everything FP64 */
     CHFSI_FP32 = 1,          /* H.X product in FP32 on fl32(Z_k); Z_k, R, Lambda_k and the recurrence stored/combined in FP64 */
-    CHFSI_TF32 = 2,          /* reserved: returns CHFSI_EUNSUPPORTED in this build */
-    CHFSI_TF32X3 = 3,        /* reserved: returns CHFSI_EUNSUPPORTED in this build */
+    CHFSI_TF32 = 2,          /* FP32-stored multivectors (as CHFSI_FP32_STORED) with the S2 cell contractions on TF32 tensor cores
+                                ("TF32 tensor operations"): operands rounded cvt.rna.tf32.f32, FP32 accumulate;
+                                pointwise terms, phases and the update stay FP32/FP64.  chfsi_cheb_filter, RESIDUAL, even p. */
+    CHFSI_TF32X3 = 3,        /* the same with the hi/lo split of both operands and three tensor-core products per
+                                contraction (small terms first): FP32-level accuracy on the tensor pipe */
     CHFSI_FP32_STORED = 4    /* the paper's layout: the multivectors Z_k themselves are complex64 inside the
                                 filter ("extraction, scatter/gather, and assembly kernels ... operate on FP32 multivectors,
                                 halving global memory traffic"), FP32 arithmetic; "only the eigenproblem residual R and the
                                 eigenvalue recurrence Lambda_k are retained in FP64", as are S0 and the recover step S7.
                                 chfsi_cheb_filter with CHFSI_RECUR_RESIDUAL and even p only (EUNSUPPORTED otherwise). */
 } chfsi_prec;
+
+/* Implementation of the dominant (cell) kernel, see chfsi_mesh_set_cell_kernel. */
+typedef enum {
+    CHFSI_CELL_DEFAULT = 0,  /* the library's choice for this precision and degree */
+    CHFSI_CELL_XYZ = 1,      /* line-owned FMA kernel (cell_xyz.cu) */
+    CHFSI_CELL_MARCH = 2,    /* plane-march FMA kernel (cell_march.cu), FP64 */
+    CHFSI_CELL_MMA = 3       /* tensor-core kernel (cell_mma.cu): mma.sync FP64 / TF32 */
+} chfsi_cell_kernel;
 
 typedef enum {
     CHFSI_RECUR_STANDARD = 0,   /* eq. 10 */
@@ -79,6 +90,10 @@ typedef enum {
 chfsi_status chfsi_mesh_create(int ncx, int ncy, int ncz, double Lx, double Ly, double Lz, int p,
                                const double* kfrac, int device, chfsi_mesh** out);
 chfsi_status chfsi_mesh_destroy(chfsi_mesh* mesh);          /* NULL is allowed */
+/* Selects which implementation of the cell kernel later calls use for precision `prec` (a plain argument, there is no
+ * environment switch); every implementation computes the same operation to the precision's tolerance.  A choice that is
+ * not built for the degree / precision / call falls back to the default at launch.  EINVAL: NULL mesh, bad enums. */
+chfsi_status chfsi_mesh_set_cell_kernel(chfsi_mesh* mesh, chfsi_prec prec, chfsi_cell_kernel kernel);
 
 /* Queries (host outputs).  nnodes = M = N1x*N1y*N1z.  xyz: M*3 doubles (x,y,z per node).
  * mass: M doubles, m_I = sum over the cells containing node I of w_a w_b w_c (hx hy hz / 8). */

@@ -21,7 +21,7 @@ RECUR_STANDARD, RECUR_RESIDUAL = 0, 1
 PREC = {"fp64": FP64, "fp32": FP32, "tf32": TF32, "tf32x3": TF32X3, "fp32s": FP32_STORED}
 
 EXPORTS = [
-    "chfsi_mesh_create", "chfsi_mesh_destroy", "chfsi_mesh_num_nodes", "chfsi_mesh_node_coords",
+    "chfsi_mesh_create", "chfsi_mesh_destroy", "chfsi_mesh_set_cell_kernel", "chfsi_mesh_num_nodes", "chfsi_mesh_node_coords",
     "chfsi_mesh_mass", "chfsi_ham_set", "chfsi_workspace_bytes", "chfsi_apply_H", "chfsi_cheb_filter",
     "chfsi_profile_enable", "chfsi_profile_read",
     "chfsi_bfp_stream_bytes", "chfsi_bfp_encode", "chfsi_bfp_decode", "chfsi_bfp_gather_encode",
@@ -50,6 +50,7 @@ def lib() -> C.CDLL:
     dp, ip, llp, vp = C.POINTER(C.c_double), C.POINTER(C.c_int), C.POINTER(C.c_longlong), C.c_void_p
     L.chfsi_mesh_create.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [C.c_int, dp, C.c_int, C.POINTER(vp)]
     L.chfsi_mesh_destroy.argtypes = [vp]
+    L.chfsi_mesh_set_cell_kernel.argtypes = [vp, C.c_int, C.c_int]
     L.chfsi_mesh_num_nodes.argtypes = [vp, llp]
     L.chfsi_mesh_node_coords.argtypes = [vp, dp]
     L.chfsi_mesh_mass.argtypes = [vp, dp]
@@ -102,6 +103,13 @@ def chfsi_mesh_create(ncell, L, p, kfrac=None, device=0):
 
 def chfsi_mesh_destroy(mesh):
     _check(lib().chfsi_mesh_destroy(mesh))
+
+
+CELL_DEFAULT, CELL_XYZ, CELL_MARCH, CELL_MMA = range(4)
+
+
+def chfsi_mesh_set_cell_kernel(mesh, prec, kernel):
+    _check(lib().chfsi_mesh_set_cell_kernel(mesh, int(prec), int(kernel)))
 
 
 def chfsi_mesh_num_nodes(mesh) -> int:

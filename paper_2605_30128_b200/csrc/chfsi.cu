@@ -112,6 +112,9 @@ struct WorkLayout {
     int nbuf;
     long long ldz;      // leading dimension of the two iterate buffers (complex elements)
 };
+// complex64 iterates inside eq. 11: FP32-stored FMA mode and the two tensor-core modes
+static inline bool stored32(chfsi_prec prec) { return prec == CHFSI_FP32_STORED || prec == CHFSI_TF32 || prec == CHFSI_TF32X3; }
+
 static WorkLayout work_layout(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur recur, int chunk, int degree_cap) {
     WorkLayout wl;
     wl.nbuf = recur == CHFSI_RECUR_RESIDUAL ? 3 : 1;
@@ -121,8 +124,8 @@ static WorkLayout work_layout(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur 
     wl.buf_bytes = align256((size_t)2 * m->nnodes * chunk * 16);
     // FP32-stored multivectors: R stays complex128, the two iterate buffers are complex64 with an even leading
     // dimension (16-byte row pitch for TMA)
-    wl.ldz = prec == CHFSI_FP32_STORED ? ((chunk + 1) & ~1) : chunk;
-    wl.zbuf_bytes = prec == CHFSI_FP32_STORED ? align256((size_t)2 * m->nnodes * wl.ldz * 8) : wl.buf_bytes;
+    wl.ldz = stored32(prec) ? ((chunk + 1) & ~1) : chunk;
+    wl.zbuf_bytes = stored32(prec) ? align256((size_t)2 * m->nnodes * wl.ldz * 8) : wl.buf_bytes;
     wl.total = wl.hdr_bytes + wl.coef_bytes + wl.c_bytes + wl.buf_bytes + (wl.nbuf - 1) * wl.zbuf_bytes;
     return wl;
 }
@@ -195,6 +198,13 @@ chfsi_status chfsi_mesh_create(int ncx, int ncy, int ncz, double Lx, double Ly, 
     }
     for (int a = 0; a < n; ++a) { mc.w[a] = m->w[a]; mc.wf[a] = (float)m->w[a]; }
     *out = m;
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_mesh_set_cell_kernel(chfsi_mesh* m, chfsi_prec prec, chfsi_cell_kernel kernel) {
+    if (!m) return fail(CHFSI_EINVAL, "mesh_set_cell_kernel: mesh is NULL");
+    if ((int)prec < 0 || (int)prec > 4 || (int)kernel < 0 || (int)kernel > 3) return fail(CHFSI_EINVAL, "mesh_set_cell_kernel: bad enum");
+    m->cell_kernel[(int)prec] = (int)kernel;
     return CHFSI_OK;
 }
 
@@ -394,7 +404,7 @@ chfsi_status chfsi_workspace_bytes(const chfsi_mesh* m, chfsi_prec prec, chfsi_r
     if (chunk < 1) return fail(CHFSI_EINVAL, "workspace_bytes: chunk must be >= 1");
     if (recur != CHFSI_RECUR_STANDARD && recur != CHFSI_RECUR_RESIDUAL) return fail(CHFSI_EINVAL, "workspace_bytes: bad recur");
     if (!cell_supported(m->p, prec)) return fail(CHFSI_EUNSUPPORTED, "workspace_bytes: precision not built");
-    if (prec == CHFSI_FP32_STORED && recur != CHFSI_RECUR_RESIDUAL)
+    if (stored32(prec) && recur != CHFSI_RECUR_RESIDUAL)
         return fail(CHFSI_EUNSUPPORTED, "workspace_bytes: FP32-stored multivectors need the residual recurrence (eq. 11)");
     *bytes = work_layout(m, prec, recur, chunk, kDegreeCap).total;
     return CHFSI_OK;
@@ -446,7 +456,6 @@ static chfsi_status check_common(const chfsi_mesh* m, chfsi_prec prec, int nvec,
     if (!m->ham_set) return fail(CHFSI_ESTATE, std::string(who) + ": chfsi_ham_set has not been called");
     if (prec != CHFSI_FP64 && prec != CHFSI_FP32 && prec != CHFSI_TF32 && prec != CHFSI_TF32X3 && prec != CHFSI_FP32_STORED)
         return fail(CHFSI_EINVAL, std::string(who) + ": unknown precision");
-    if (prec == CHFSI_TF32 || prec == CHFSI_TF32X3) return fail(CHFSI_EUNSUPPORTED, std::string(who) + ": TF32 paths are not built");
     if (!cell_supported(m->p, prec)) return fail(CHFSI_EUNSUPPORTED, std::string(who) + ": precision/degree not built");
     if (nvec < 1) return fail(CHFSI_EINVAL, std::string(who) + ": nvec must be >= 1");
     if (!X || !Y || !work) return fail(CHFSI_EINVAL, std::string(who) + ": NULL device pointer");
@@ -461,7 +470,7 @@ chfsi_status chfsi_apply_H(const chfsi_mesh* m, chfsi_prec prec, int nvec, const
     chfsi_status stt = check_common(m, prec, nvec, X, ldx, Y, ldy, work, "apply_H");
     if (stt != CHFSI_OK) return stt;
     if (X == Y) return fail(CHFSI_EINVAL, "apply_H: X and Y must be distinct");
-    if (prec == CHFSI_FP32_STORED) return fail(CHFSI_EUNSUPPORTED, "apply_H: FP32-stored multivectors exist only inside chfsi_cheb_filter");
+    if (stored32(prec)) return fail(CHFSI_EUNSUPPORTED, "apply_H: FP32-stored multivectors (FP32_STORED, TF32, TF32X3) exist only inside chfsi_cheb_filter");
     const size_t need = 2 * align256((size_t)(m->nl.crows > 0 ? m->nl.crows : 1) * nvec * 16);
     if (work_bytes < need) return fail(CHFSI_EINVAL, "apply_H: work_bytes too small");
     DeviceGuard g(m->device);
@@ -523,7 +532,7 @@ chfsi_status chfsi_cheb_filter(const chfsi_mesh* m, chfsi_prec prec, chfsi_recur
     if (chunk > chfsi_mesh::kStageLambda) return fail(CHFSI_EINVAL, "cheb_filter: chunk must be <= 8192 vectors");
     if (recur == CHFSI_RECUR_RESIDUAL && !lambda_host) return fail(CHFSI_EINVAL, "cheb_filter: lambda_host is NULL");
     if (X == Y && ldx != ldy) return fail(CHFSI_EINVAL, "cheb_filter: aliased X/Y need equal leading dimensions");
-    const bool st32 = prec == CHFSI_FP32_STORED;
+    const bool st32 = stored32(prec);
     if (st32 && recur != CHFSI_RECUR_RESIDUAL)
         return fail(CHFSI_EUNSUPPORTED, "cheb_filter: FP32-stored multivectors need the residual recurrence (eq. 11)");
     const WorkLayout wl = work_layout(m, prec, recur, chunk, kDegreeCap);

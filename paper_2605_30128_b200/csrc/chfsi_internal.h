@@ -113,6 +113,7 @@ struct chfsi_mesh {
     double kfrac[3] = {0, 0, 0};
     long long nnodes = 0;
     bool ham_set = false;
+    int cell_kernel[5] = {0, 0, 0, 0, 0};   // per chfsi_prec: chfsi_cell_kernel choice (0 = default)
     chfsi::MeshConst mc;
     std::vector<double> xi, w;          // host GLL tables
     std::vector<double> m1h[3];         // host assembled 1-D mass per global line index
@@ -168,6 +169,9 @@ cudaError_t launch_cell_march(const chfsi_mesh* m, chfsi_prec prec, const CellAr
 // line-owned x/y/z TMA kernel (cell_xyz.cu)
 bool xyz_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
 cudaError_t launch_cell_xyz(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
+// tensor-core cell kernel (cell_mma.cu): mma.sync TF32 / 3xTF32 on complex64 storage, mma.sync FP64 on complex128 storage
+bool mma_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
+cudaError_t launch_cell_mma(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
 void set_error(const std::string& s);
 void count_launch(int n = 1);
 }  // namespace chfsi

@@ -519,6 +519,7 @@ static cudaError_t launch_cell_t(const chfsi_mesh* m, const CellArgs& a, cudaStr
 
 bool cell_supported(int p, chfsi_prec prec) {
     if (prec == CHFSI_FP32_STORED) return p == 2 || p == 4 || p == 6 || p == 8;   // line-owned kernel only
+    if (prec == CHFSI_TF32 || prec == CHFSI_TF32X3) return p == 2 || p == 4 || p == 6 || p == 8;   // tensor-core kernel only
     if (prec != CHFSI_FP64 && prec != CHFSI_FP32) return false;
     return p >= 1 && p <= 8;
 }
@@ -535,8 +536,14 @@ cudaError_t launch_cell(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a,
         cudaEventRecord(e0, st);
     }
     cudaError_t err;
-    const bool use_march = prec == CHFSI_FP64 && m->p <= 6 && march_supported(m, prec, a);
-    if (!use_march && xyz_supported(m, prec, a)) err = launch_cell_xyz(m, prec, a, st);
+    const int choice = m->cell_kernel[(int)prec];             // chfsi_mesh_set_cell_kernel; 0 = the library's choice
+    const bool tf = prec == CHFSI_TF32 || prec == CHFSI_TF32X3;
+    const bool use_mma = (tf || (prec == CHFSI_FP64 && choice == CHFSI_CELL_MMA)) && mma_supported(m, prec, a);
+    const bool use_march = !use_mma && prec == CHFSI_FP64 && (choice == CHFSI_CELL_MARCH || (choice == 0 && m->p <= 6)) &&
+                           march_supported(m, prec, a);
+    if (use_mma) err = launch_cell_mma(m, prec, a, st);
+    else if (tf) err = cudaErrorInvalidValue;
+    else if (!use_march && xyz_supported(m, prec, a)) err = launch_cell_xyz(m, prec, a, st);
     else if (use_march) err = launch_cell_march(m, prec, a, st);
     else if (a.store_f32) err = cudaErrorInvalidValue;
     else err = launch_cell_legacy(m, prec, a, st);

@@ -16,6 +16,7 @@ from paper_2605_30128_b200 import inputs as inp
 
 sys.path.insert(0, os.path.dirname(__file__))
 from test_gpu_parity import Problem, relerr, TOL64, TOL32, TOL32S  # noqa: E402
+TOL_TF32 = 5e-3   # single-pass TF32 per filter call; the eigenvalue criterion is what it is held to
 
 pytestmark = pytest.mark.gpu
 
@@ -107,16 +108,15 @@ def test_config2_full_size_fp32_product(case_c2, env):
 
 @pytest.mark.parametrize("nvec", [64, 128, 256, 1024])
 def test_config4_sweep_nvec_and_precision(case_c2, env, nvec):
-    """configs[4]: config 2's mesh, N_vec in {64,...,1024} x {FP64, FP32} (512 is the test above; the TF32 modes
-    return CHFSI_EUNSUPPORTED, A7).  1024 vectors run in chunks of 256 so the workspace fits."""
+    """configs[4]: config 2's mesh, N_vec in {64,...,1024} x {FP64, FP32 product, FP32 stored, 3xTF32, TF32} (512 is the
+    test above).  1024 vectors run in chunks of 256 so the workspace fits."""
     torch, _, B = env
     pos = [0, nvec // 3, nvec // 2 + 1, nvec - 1]
     chunk = 256 if nvec > 512 else 0
     ref4 = case_c2.ref[:, :, :4]                       # the first four seeded columns, placed at `pos`
-    for prec, tol, name in [(B.FP64, TOL64, "fp64"), (B.FP32, TOL32, "fp32"), (B.FP32_STORED, TOL32S, "fp32s")]:
+    for prec, tol, name in [(B.FP64, TOL64, "fp64"), (B.FP32, TOL32, "fp32"), (B.FP32_STORED, TOL32S, "fp32s"),
+                            (B.TF32X3, TOL32, "tf32x3"), (B.TF32, TOL_TF32, "tf32")]:
         check(case_c2.run(nvec, pos, prec, chunk=chunk, ncols=4), ref4, tol, f"c4 nvec={nvec} {name}")
-    with pytest.raises(Exception):
-        case_c2.run(64, [0, 1, 2, 3], B.TF32, ncols=4)
 
 
 def test_config3_full_size_p8_bloch_chunked(env):
