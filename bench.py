@@ -38,8 +38,11 @@ METRIC = "chebyshev_filter_throughput"
 UNIT = "complex_DoF*vectors*degree/s"
 FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md fallback
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_cell_kernel_traffic.csv")
-DTYPE = {"fp64": "f64", "fp32": "f32 product / f64 storage and recurrence",
-         "fp32s": "f32 multivectors / f64 residual and Lambda_k"}
+DTYPE = {"fp64": "f64", "fp64m": "f64 (cell contractions on mma.sync.m8n8k4.f64)",
+         "fp32": "f32 product / f64 storage and recurrence",
+         "fp32s": "f32 multivectors / f64 residual and Lambda_k",
+         "tf32": "f32 multivectors, tf32 tensor-core cell contractions / f64 residual and Lambda_k",
+         "tf32x3": "f32 multivectors, 3xtf32 tensor-core cell contractions / f64 residual and Lambda_k"}
 
 
 def measured_hbm_peak():
@@ -120,7 +123,7 @@ def alg_bytes_per_unit(prec, recur="residual"):
     ("only R and Lambda_k in FP64"): 8 + 16 + 16 = 40 B.  eq. 10: no R, 48 B."""
     if recur != "residual":
         return 48.0
-    return 40.0 if prec == "fp32s" else 64.0
+    return 40.0 if prec in ("fp32s", "tf32", "tf32x3") else 64.0
 
 
 # --------------------------------------------------------------------------------------------
@@ -182,7 +185,8 @@ class Workload:
     def __init__(self, torch, B, cfg, prec_name, recur_name, nvec, device, seed, pb=None):
         from paper_2605_30128_b200.harness import GpuProblem
         self.torch, self.B, self.cfg = torch, B, cfg
-        self.prec = B.PREC[prec_name]
+        self.prec = B.PREC["fp64" if prec_name == "fp64m" else prec_name]
+        self.mma64 = prec_name == "fp64m"        # FP64 on the tensor-core cell kernel (chfsi_mesh_set_cell_kernel)
         self.recur = B.RECUR_RESIDUAL if recur_name == "residual" else B.RECUR_STANDARD
         self.nvec = nvec
         self.chunk = cfg.chunk if (cfg.chunk and cfg.chunk < nvec) else (256 if nvec > 512 else 0)
@@ -203,6 +207,9 @@ class Workload:
         self.stream = torch.cuda.current_stream()
 
     def step(self):
+        if self.mma64 != getattr(self.pb, "_mma64", False):
+            self.B.chfsi_mesh_set_cell_kernel(self.pb.mesh, self.B.FP64, self.B.CELL_MMA if self.mma64 else self.B.CELL_DEFAULT)
+            self.pb._mma64 = self.mma64
         self.B.chfsi_cheb_filter(self.pb.mesh, self.prec, self.recur, self.cfg.degree, self.a, self.b, self.a0, self.X,
                                  self.lam, self.Y, self.work, chunk=self.chunk, stream=self.stream)
 
@@ -293,8 +300,8 @@ def all_configs_table(torch, B, device, peak):
         rows.append(row)
     finally:
         w.close()
-    for cfg_id, precs, nvecs in [(1, ["fp64", "fp32", "fp32s"], [128]), (3, ["fp64", "fp32", "fp32s"], [256]),
-                                 (4, ["fp64", "fp32", "fp32s"], [64, 128, 256, 512, 1024])]:
+    ALLP = ["fp64", "fp64m", "fp32", "fp32s", "tf32x3", "tf32"]
+    for cfg_id, precs, nvecs in [(1, ALLP, [128]), (3, ALLP, [256]), (4, ALLP, [64, 128, 256, 512, 1024])]:
         cfg = inp.CONFIGS[cfg_id]
         pb = GpuProblem(cfg, seed=0, device=device)
         try:
@@ -504,7 +511,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
-    ap.add_argument("--prec", default=None, choices=["fp64", "fp32", "fp32s"])
+    ap.add_argument("--prec", default=None, choices=["fp64", "fp64m", "fp32", "fp32s", "tf32", "tf32x3"])
     ap.add_argument("--recur", default="residual", choices=["residual", "standard"])
     ap.add_argument("--nvec", type=int, default=0)
     ap.add_argument("--ref-cols", type=int, default=0, help="columns in the CPU-oracle sample")

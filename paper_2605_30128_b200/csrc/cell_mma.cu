@@ -6,24 +6,30 @@
 // per unit in the FP32-stored mode, 39 % with 2.7 warps per scheduler in FP64 -- so the lever is instructions per unit,
 // not flops.  One mma.sync.m16n8k8.tf32 replaces 32 FFMA warp instructions, one mma.sync.m8n8k4.f64 eight DFMA ones.
 // (tcgen05.mma was evaluated and rejected for this contraction: its A operand must be the data tile, M = 128 rows by
-// K = 8 deep from shared memory, 4 KB per instruction for a 9-wide B; at the measured ~128 B/clk of operand bandwidth that
-// is >= 32 clk per instruction, 3.9 kclk per plane and contraction pass against a 1.8 kclk HBM budget -- DESIGN.md 6.5.)
+// K = 8 deep from shared memory, 4 KB per instruction for a 9-wide B; at ~128 B/clk of operand bandwidth that is >= 32 clk
+// per instruction, 3.9 kclk per plane and contraction pass against a 1.8 kclk HBM budget -- DESIGN.md 6.5.)
 //
 // Formulation.  For each direction the contraction is  D[col][out] = sum_in A[col][in] B[in][out]  with
 //   A = the data (M = the CTA's real batch columns of one spin component: 16 for TF32, 8 for FP64; K = the p+1 nodes of a
 //       line), loaded as fragments straight from the TMA-landed plane in shared memory,
-//   B = the (p+1) x (p+1) 1-D operator, transposed, held as fragments in registers for the whole kernel.
+//   B = ONE (p+1) x (p+1) matrix for all three directions (on this mesh the scaled 1-D operators differ by a scalar),
+//       transposed, held as fragments in registers for the whole kernel.
 // A CTA owns the xy-footprint of one cell column, a z-segment and C real batch columns, and marches through the planes:
-//   X task (warp = row j, spin):   x-contraction of row j of plane t+1        -> shared XR (one plane ahead)
-//   Y task (warp = x-position i):  y-contraction at x-position i of plane t, + XR, + S5 on owned nodes -> RED to `out`
+//   X task (warp = row j, spin):   x-contraction of row j of plane t+1, + S5 on owned nodes   -> shared XR (one plane ahead)
+//   Y task (warp = x-position i):  y-contraction at x-position i of plane t, + XR             -> RED to `out`
 //   Z task (at the end of a cell): z-contraction over the p+1 planes of the cell, which are all resident in the plane
-//                                  ring (no z accumulators in registers), for the warp's row of nodes    -> RED to `out`
+//                                  ring (no z accumulators in registers), for the warp's row of nodes -> RED to `out`
 // D comes out as (column g, outputs 2t, 2t+1): eight lanes hold eight adjacent columns, so every RED covers full 32-byte
 // sectors.  An output node receives two REDs (in-plane part + S5, z part) instead of one.
-// Modes: MM_F64 (complex128 storage, mma.m8n8k4.f64), MM_TF32 (complex64 storage, operands rounded cvt.rna.tf32.f32, FP32
-// accumulate: CHFSI_TF32), MM_TF32X3 (hi/lo split of both operands, three MMAs, small terms first: CHFSI_TF32X3).
+// Shared-memory layout: a plane is [p+1 lines][p+1 nodes][128 B] (the x = P face column sits inline as node P of its line),
+// landed by TMA with the 128-byte swizzle; fragment loads whose four k-lanes differ in node, line or plane then hit
+// distinct banks (the plane pitch is 2 mod 8 rows of 128 B, the ring has a multiple of 4 slots, k is interleaved 2t, 2t+1).
+// Modes: MM_F64 (complex128 storage, mma.m8n8k4.f64), MM_TF32 (complex64 storage, operands rounded to TF32 by
+// round-to-nearest-away, FP32 accumulate: CHFSI_TF32), MM_TF32X3 (hi/lo split of both operands, three MMAs, small terms
+// first: CHFSI_TF32X3).
 #include <cuda.h>
 
+#include <cmath>
 #include <cstring>
 #include <mutex>
 #include <type_traits>
@@ -40,10 +46,13 @@ template <> struct MmaTraits<MM_F64> { using T = double; static constexpr int MR
 
 template <typename T>
 struct MmaConst {
-    T K[3][kMaxN][kMaxN];       // scaled 1-D operators K[d][out][in] (all scalings folded in, see build_mma_const)
+    T K[kMaxN][kMaxN];          // base 1-D operator K[out][in]: the z-direction operator with its scalings folded in
     T W[3][kMaxN];              // WX, WY, WZ
+    T sdir[3];                  // operator of direction d = sdir[d] * K   (sdir[2] = 1)
     double cHp;                 // coefficient of the potential term
 };
+
+constexpr bool kSwizzle = false; // 128-byte TMA swizzle of the plane and R stages (false: linear layout, for debugging)
 
 template <int P, int MODE>
 struct MmaCfg {
@@ -51,38 +60,45 @@ struct MmaCfg {
     static constexpr int n = P + 1;
     static constexpr int MROWS = MmaTraits<MODE>::MROWS, KSTEP = MmaTraits<MODE>::KSTEP;
     static constexpr int C = 2 * MROWS, NV = C / 4;          // real batch columns of the CTA: both spin components
-    static constexpr int NR = MROWS / 8, KH = KSTEP / 4;     // fragment rows g + 8r, fragment k-halves t + 4h
+    static constexpr int NR = MROWS / 8, KH = KSTEP / 4;     // fragment rows g + 8r, fragment k-halves
     static constexpr int KS = (n + KSTEP - 1) / KSTEP, NT = (n + 7) / 8;
     static constexpr int NCW = 2 * n;                        // consumer warps: (index q in 0..p) x (spin)
     static constexpr int THREADS = (NCW + 1) * 32;
     static constexpr int ESZ = (int)sizeof(T);
-    // plane ring stage: MAIN [n lines][P nodes][C] | FACE [n lines][C] (the x = P column)
-    static constexpr int FACE_ELEMS = n * P * C;
-    static constexpr int IN_BYTES = n * n * C * ESZ;
-    static constexpr int IN_STAGE = ((IN_BYTES + 127) / 128) * 128;
-    // R / fields ring stage: R [P][P][C] f64 | fields [P][P][4] f64
+    static_assert(C * ESZ == 128, "one node of the CTA's columns is one 128-byte row");
+    // plane ring stage: [n lines][n nodes][128 B]; pitch = n^2 + 1 rows of 128 B (n odd => n^2 = 1 mod 8 => pitch = 2 mod 8)
+    static constexpr int LINE_BYTES = n * 128;
+    static constexpr int IN_BYTES = n * n * 128;
+    static constexpr int IN_STAGE = (n * n + 1) * 128;
+    // R / fields ring stage: R [P lines][P nodes][2 spins][C/2 doubles] | fields [P][P][4] f64
     static constexpr int R_BYTES = P * P * C * 8, F_BYTES = P * P * 32;
-    static constexpr int R_STAGE = ((R_BYTES + F_BYTES + 127) / 128) * 128;
+    static constexpr int R_STAGE = ((R_BYTES + F_BYTES + 1023) / 1024) * 1024;
     static constexpr int RS = 3;
     // XR[row][x'][XP]: the x-contraction of a plane, column pitch padded by 16 bytes (bank spread of the fragment accesses)
     static constexpr int XP = C + 16 / ESZ;
     static constexpr int XR_BYTES = ((n * n * XP * ESZ + 127) / 128) * 128;
-    static constexpr int S_ = (220 * 1024 - 2 * XR_BYTES - RS * R_STAGE) / IN_STAGE;
+    static constexpr int S_ = ((219 * 1024 - 2 * XR_BYTES - RS * R_STAGE) / IN_STAGE) / 4 * 4;     // a multiple of 4 slots
     static constexpr int S = S_ < 16 ? S_ : 16;
     static_assert(S >= P + 2, "plane ring must hold a whole cell plus the plane ahead");
-    static constexpr size_t SMEM = (size_t)S * IN_STAGE + (size_t)RS * R_STAGE + 2 * (size_t)XR_BYTES;
+    static constexpr int R_OFF = ((S * IN_STAGE + 1023) / 1024) * 1024;
+    static constexpr int XR_OFF = R_OFF + RS * R_STAGE;
+    static constexpr size_t SMEM = (size_t)XR_OFF + 2 * (size_t)XR_BYTES + 1024;   // + slack to align the base to 1024 B
 };
+
+// byte offset (from the 1024-aligned base) -> swizzled byte offset: the 16-byte chunk index (bits 4..6) is XORed with the
+// 128-byte row index (bits 7..9), which is what CU_TENSOR_MAP_SWIZZLE_128B does to the bytes TMA writes
+__device__ __forceinline__ uint32_t swz(uint32_t lin) { return kSwizzle ? lin ^ ((lin >> 3) & 0x70u) : lin; }
 
 __device__ __forceinline__ void red_add_t(double* p, double v) { atomicAdd(p, v); }     // result unused -> RED
 __device__ __forceinline__ void red_add_t(float* p, float v) { atomicAdd(p, v); }
 
-__device__ __forceinline__ uint32_t to_tf32(float x) {
-    uint32_t r;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-    return r;
-}
+// round-to-nearest, ties away from zero, to the 10-bit TF32 mantissa (what cvt.rna.tf32.f32 returns for finite inputs):
+// add half an ulp of TF32 to the magnitude bits; the tensor core ignores the low 13 bits
+__device__ __forceinline__ uint32_t to_tf32(float x) { return __float_as_uint(x) + 0x1000u; }
+__device__ __forceinline__ float tf32_value(uint32_t b) { return __uint_as_float(b & 0xffffe000u); }
+
 __device__ __forceinline__ void mma_tf32(float (&d)[2][2], const uint32_t (&a)[2][2], const uint32_t (&b)[2]) {
-    // a[r][h] = A(row g + 8r, k = t + 4h) -> a0 = a[0][0], a1 = a[1][0], a2 = a[0][1], a3 = a[1][1]; d[r][e] = D(row g + 8r, col 2t + e)
+    // a[r][h] = A(row g + 8r, k-half h) -> a0 = a[0][0], a1 = a[1][0], a2 = a[0][1], a3 = a[1][1]; d[r][e] = D(row g + 8r, col 2t + e)
     asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+f"(d[0][0]), "+f"(d[0][1]), "+f"(d[1][0]), "+f"(d[1][1])
                  : "r"(a[0][0]), "r"(a[1][0]), "r"(a[0][1]), "r"(a[1][1]), "r"(b[0]), "r"(b[1]));
@@ -92,34 +108,41 @@ __device__ __forceinline__ void mma_f64(double (&d)[1][2], double a, double b) {
                  : "+d"(d[0][0]), "+d"(d[0][1]) : "d"(a), "d"(b));
 }
 
-// B fragments of the three 1-D operators, per thread: B[k = in][n = out] = K[out][in]
+// The line index that fragment position (k-step ks, half h, lane t) contracts over.  TF32: k = t and k = t + 4 of a k-step are
+// mapped to the neighbouring nodes 2t and 2t+1, so that the four lanes of a load differ in bits 1..2 of the 128-byte row
+// index and the swizzle spreads them over all banks.  Any permutation is legal as long as A and B use the same one.
+template <int MODE>
+__device__ __forceinline__ int kmap(int ks, int h, int t) {
+    return MODE == MM_F64 ? ks * 4 + t : ks * 8 + 2 * t + h;
+}
+
+// B fragments of the base 1-D operator, per thread: B[k = in][n = out] = K[out][in]
 template <int P, int MODE>
 struct BFrags {
     using Cfg = MmaCfg<P, MODE>;
     using T = typename Cfg::T;
     using TB = typename std::conditional<MODE == MM_F64, double, uint32_t>::type;
-    TB hi[3][Cfg::KS][Cfg::NT][Cfg::KH];
-    TB lo[MODE == MM_TF32X3 ? 3 : 1][Cfg::KS][Cfg::NT][Cfg::KH];
+    TB hi[Cfg::KS][Cfg::NT][Cfg::KH];
+    TB lo[MODE == MM_TF32X3 ? Cfg::KS : 1][Cfg::NT][Cfg::KH];
 
     __device__ __forceinline__ void init(const MmaConst<T>& sc, int g, int t) {
 #pragma unroll
-        for (int d = 0; d < 3; ++d)
+        for (int ks = 0; ks < Cfg::KS; ++ks)
 #pragma unroll
-            for (int ks = 0; ks < Cfg::KS; ++ks)
+            for (int nt = 0; nt < Cfg::NT; ++nt)
 #pragma unroll
-                for (int nt = 0; nt < Cfg::NT; ++nt)
-#pragma unroll
-                    for (int h = 0; h < Cfg::KH; ++h) {
-                        const int out = nt * 8 + g, in = ks * Cfg::KSTEP + t + 4 * h;
-                        const T v = (out < Cfg::n && in < Cfg::n) ? sc.K[d][out < Cfg::n ? out : 0][in < Cfg::n ? in : 0] : (T)0;
-                        if constexpr (MODE == MM_F64) {
-                            hi[d][ks][nt][h] = v;
-                        } else {
-                            const uint32_t vh = to_tf32(v);
-                            hi[d][ks][nt][h] = vh;
-                            if constexpr (MODE == MM_TF32X3) lo[d][ks][nt][h] = to_tf32(v - __uint_as_float(vh));
-                        }
+                for (int h = 0; h < Cfg::KH; ++h) {
+                    const int out = nt * 8 + g, in = kmap<MODE>(ks, h, t);
+                    const bool ok = out < Cfg::n && in < Cfg::n;
+                    const T v = ok ? sc.K[ok ? out : 0][ok ? in : 0] : (T)0;
+                    if constexpr (MODE == MM_F64) {
+                        hi[ks][nt][h] = v;
+                    } else {
+                        const uint32_t vh = to_tf32(v);
+                        hi[ks][nt][h] = vh;
+                        if constexpr (MODE == MM_TF32X3) lo[ks][nt][h] = to_tf32(v - tf32_value(vh));
                     }
+                }
     }
 };
 
@@ -135,9 +158,8 @@ struct Acc {
     }
 };
 
-// acc += (operator of direction DIR) applied along the line whose element kk = KSTEP ks + t + 4 h (0..p) for fragment row r
-// is ld(ks, h, kk, r)
-template <int P, int MODE, int DIR, typename LD>
+// acc += K applied along the line whose element kmap(ks, h, t) for fragment row r is ld(ks, h, r)
+template <int P, int MODE, typename LD>
 __device__ __forceinline__ void contract(Acc<P, MODE>& acc, const BFrags<P, MODE>& bf, int t, LD ld) {
     using Cfg = MmaCfg<P, MODE>;
     using T = typename Cfg::T;
@@ -146,15 +168,15 @@ __device__ __forceinline__ void contract(Acc<P, MODE>& acc, const BFrags<P, MODE
         T a[Cfg::NR][Cfg::KH];
 #pragma unroll
         for (int h = 0; h < Cfg::KH; ++h) {
-            const int kk = ks * Cfg::KSTEP + t + 4 * h;
             // the last k-step is only partly populated: lanes beyond the line contribute zeros
-            const bool ok = (ks * Cfg::KSTEP + 3 + 4 * h < Cfg::n) || kk < Cfg::n;
+            const bool all = kmap<MODE>(ks, h, 3) < Cfg::n;
+            const bool ok = all || kmap<MODE>(ks, h, t) < Cfg::n;
 #pragma unroll
-            for (int r = 0; r < Cfg::NR; ++r) a[r][h] = ok ? ld(ks, h, kk, r) : (T)0;
+            for (int r = 0; r < Cfg::NR; ++r) a[r][h] = ok ? ld(ks, h, r) : (T)0;
         }
         if constexpr (MODE == MM_F64) {
 #pragma unroll
-            for (int nt = 0; nt < Cfg::NT; ++nt) mma_f64(acc.d[nt], a[0][0], bf.hi[DIR][ks][nt][0]);
+            for (int nt = 0; nt < Cfg::NT; ++nt) mma_f64(acc.d[nt], a[0][0], bf.hi[ks][nt][0]);
         } else {
             uint32_t ah[2][2], al[2][2];
 #pragma unroll
@@ -162,34 +184,37 @@ __device__ __forceinline__ void contract(Acc<P, MODE>& acc, const BFrags<P, MODE
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     ah[r][h] = to_tf32(a[r][h]);
-                    if constexpr (MODE == MM_TF32X3) al[r][h] = to_tf32(a[r][h] - __uint_as_float(ah[r][h]));
+                    if constexpr (MODE == MM_TF32X3) al[r][h] = to_tf32(a[r][h] - tf32_value(ah[r][h]));
                 }
 #pragma unroll
             for (int nt = 0; nt < Cfg::NT; ++nt) {
                 if constexpr (MODE == MM_TF32X3) {
-                    mma_tf32(acc.d[nt], al, bf.hi[DIR][ks][nt]);       // small terms first
-                    mma_tf32(acc.d[nt], ah, bf.lo[DIR][ks][nt]);
+                    mma_tf32(acc.d[nt], al, bf.hi[ks][nt]);            // small terms first
+                    mma_tf32(acc.d[nt], ah, bf.lo[ks][nt]);
                 }
-                mma_tf32(acc.d[nt], ah, bf.hi[DIR][ks][nt]);
+                mma_tf32(acc.d[nt], ah, bf.hi[ks][nt]);
             }
         }
     }
 }
 
-template <int P, int MODE, bool HASPH>
+template <int P, int MODE, bool HASPH, bool FULLV>
 __global__ void __launch_bounds__(MmaCfg<P, MODE>::THREADS, 1)
 cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc, const __grid_constant__ MarchArgs ar,
                 const __grid_constant__ MarchMaps mp) {
     using Cfg = MmaCfg<P, MODE>;
     using T = typename Cfg::T;
+    using T2 = typename std::conditional<MODE == MM_F64, double2, float2>::type;
     constexpr int n = Cfg::n, C = Cfg::C, S = Cfg::S, RS = Cfg::RS, XP = Cfg::XP, NR = Cfg::NR, NT = Cfg::NT, MROWS = Cfg::MROWS;
-    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int ESZ = Cfg::ESZ, KS = Cfg::KS, KH = Cfg::KH;
+    extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t full_in[S], empty_in[S], full_r[RS], empty_r[RS];
-    unsigned char* rring = smem + (size_t)S * Cfg::IN_STAGE;
-    T* XRb = reinterpret_cast<T*>(rring + (size_t)RS * Cfg::R_STAGE);
+    // the swizzle is a function of shared-memory address bits 4..9: work from a 1024-byte aligned base
+    unsigned char* const smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    T* const XRb = reinterpret_cast<T*>(smem + Cfg::XR_OFF);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    constexpr int ROWB = (C / 2) * Cfg::ESZ;
+    constexpr int ROWB = (C / 2) * ESZ;
     constexpr int PAIR = ROWB >= 128 ? 1 : 128 / ROWB;
     int bid = blockIdx.x;
     const int cpair = bid % PAIR; bid /= PAIR;
@@ -215,67 +240,92 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
             const int col0 = chunk * (C / 2);
             uint64_t pol_last;
             asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_last));
+            int s = 0, rs = 0, ps = 0, prs = 0;               // ring slots and their phase parities
             for (int t = 0; t < T_; ++t) {
-                const int s = t % S;
-                mbar_wait(&empty_in[s], ((t / S) & 1) ^ 1);
+                mbar_wait(&empty_in[s], ps ^ 1);
                 mbar_expect_tx(&full_in[s], Cfg::IN_BYTES);
                 unsigned char* st = smem + (size_t)s * Cfg::IN_STAGE;
                 int gz = g0 + t; if (gz == ar.n1[2]) gz = 0;
-                const int line = gz * ar.n1[1] + ey * P;
-                const int xr = 2 * ex * P;
-                const int xf = xwrap ? 0 : xr + 2 * P;
-                if (!ywrap) {
-                    tma_load_3d(st, &mp.main[0], col0, xr, line, &full_in[s]);
-                    tma_load_3d(st + Cfg::FACE_ELEMS * Cfg::ESZ, &mp.face[0], col0, xf, line, &full_in[s]);
+                const int line = gz * ar.n1[1] + ey * P;        // first x-line of the footprint in plane gz
+                const int wline = gz * ar.n1[1];                // the y-wrapped line P of the last cell row
+                const int xr = 2 * ex * P;                      // first (node, spin) row of the cell in its x-line
+                if (!xwrap) {
+                    // the face column x = P is the next node of every line: one box of 2(P+1) rows per line
+                    if (!ywrap) {
+                        tma_load_3d(st, &mp.main[0], col0, xr, line, &full_in[s]);
+                    } else {
+                        tma_load_3d(st, &mp.main[1], col0, xr, line, &full_in[s]);
+                        tma_load_3d(st + P * Cfg::LINE_BYTES, &mp.main[2], col0, xr, wline, &full_in[s]);
+                    }
                 } else {
-                    tma_load_3d(st, &mp.main[1], col0, xr, line, &full_in[s]);
-                    tma_load_3d(st + P * P * C * Cfg::ESZ, &mp.main[2], col0, xr, gz * ar.n1[1], &full_in[s]);
-                    tma_load_3d(st + Cfg::FACE_ELEMS * Cfg::ESZ, &mp.face[1], col0, xf, line, &full_in[s]);
-                    tma_load_3d(st + (Cfg::FACE_ELEMS + P * C) * Cfg::ESZ, &mp.face[2], col0, xf, gz * ar.n1[1], &full_in[s]);
+                    // last cell in x: node P of a line is the line's node 0 -- per line, 2P rows and then the 2 wrapped rows
+                    for (int j = 0; j < n; ++j) {
+                        const int gl = (j == P && ywrap) ? wline : line + j;
+                        tma_load_3d(st + j * Cfg::LINE_BYTES, &mp.face[0], col0, xr, gl, &full_in[s]);
+                        tma_load_3d(st + j * Cfg::LINE_BYTES + P * 128, &mp.face[1], col0, 0, gl, &full_in[s]);
+                    }
                 }
-                if (t < T_ - 1) {                              // owned plane: R and the packed fields for S5
-                    const int rs = t % RS;
-                    mbar_wait(&empty_r[rs], ((t / RS) & 1) ^ 1);
+                if (t < T_ - 1) {                               // owned plane: R and the packed fields for S5
+                    mbar_wait(&empty_r[rs], prs ^ 1);
                     mbar_expect_tx(&full_r[rs], Cfg::F_BYTES + (ar.useR ? Cfg::R_BYTES : 0));
-                    unsigned char* rt = rring + (size_t)rs * Cfg::R_STAGE;
-                    if (ar.useR) tma_load_3d(rt, &mp.R, chunk * (C / 2), xr, line, &full_r[rs]);
+                    unsigned char* rt = smem + Cfg::R_OFF + (size_t)rs * Cfg::R_STAGE;
+                    if (ar.useR) tma_load_3d(rt, &mp.R, col0, xr, line, &full_r[rs]);
                     tma_load_2d_hint(rt + Cfg::R_BYTES, &mp.F, 4 * ex * P, line, &full_r[rs], pol_last);
+                    if (++rs == RS) { rs = 0; prs ^= 1; }
                 }
+                if (++s == S) { s = 0; ps ^= 1; }
             }
         }
         return;
     }
 
     // ================================ consumers ================================
-    const int mt = warp & 1, q = warp >> 1;       // spin component (= m-tile), index: row j (X, Z tasks) / x-position i (Y task)
+    const int mt = warp & 1, q = warp >> 1;       // spin component (= m-tile); index: row j (X, Z tasks) / x-position i (Y task)
     const int g = lane >> 2, t4 = lane & 3;
     const int col0 = mt * MROWS + g;              // fragment row r is column col0 + 8 r
+    const uint32_t fb0 = (uint32_t)col0 * ESZ;    // its byte offset inside a node's 128-byte row
     const int ri = g & 1;
     const double sg = ((ri == 0) != (mt == 0)) ? -1.0 : 1.0;
+    const int NTH = Cfg::NCW * 32;
     BFrags<P, MODE> bf;
     bf.init(sc, g, t4);
     bool vok[NR];
     double cin[NR], cR[NR];
-    long long ocol[NR];                           // scalar offset of the thread's column inside a node's 4 ld scalars
+    int v0 = 0;
 #pragma unroll
     for (int r = 0; r < NR; ++r) {
-        const int vl = (8 * r + g) >> 1;
-        const int v = chunk * Cfg::NV + vl;
-        vok[r] = v < ar.nvec;
+        const int v = chunk * Cfg::NV + ((8 * r + g) >> 1);
+        vok[r] = FULLV || v < ar.nvec;
+        if (r == 0) v0 = v;
         cin[r] = (vok[r] && ar.cin) ? __ldg(ar.cin + v) : 0.0;
         cR[r] = (vok[r] && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
-        ocol[r] = ((long long)mt * ar.ld_out + (vok[r] ? v : 0)) * 2 + ri;
     }
+    // `out` offsets in scalars of T: node I -> 4 ld I; spin -> 2 ld; vector v -> 2 v; fragment row r = 1 is 4 vectors on
     const long long XS = 4 * ar.ld_out, LS = (long long)ar.n1[0] * XS, PS = (long long)ar.n1[1] * LS;
+    const long long ocol0 = ((long long)mt * ar.ld_out + (FULLV || v0 < ar.nvec ? v0 : 0)) * 2 + ri;
     T* const outp = reinterpret_cast<T*>(ar.out);
-    const bool xph = HASPH && xwrap && ar.phd[0], yph = HASPH && ywrap && ar.phd[1];
-    const T WXq = sc.W[0][q], WYq = sc.W[1][q];
-    // node offsets of the footprint: x-position i / line j of this cell column, wrapped
     auto xoff = [&](int i) { int gx = ex * P + i; if (gx == ar.n1[0]) gx = 0; return (long long)gx * XS; };
     auto yoff = [&](int j) { int gy = ey * P + j; if (gy == ar.n1[1]) gy = 0; return (long long)gy * LS; };
     auto zoff = [&](int gzp) { if (gzp == ar.n1[2]) gzp = 0; return (long long)gzp * PS; };
-    auto stage = [&](int tp) { return reinterpret_cast<T*>(smem + (size_t)(tp % S) * Cfg::IN_STAGE); };
-    const int NTH = Cfg::NCW * 32;
+    // this thread's output rows: 2 t4 + e of the first n-tile, and row 8 + 2 t4 + e of the second (live only where < n)
+    const long long yq0 = yoff(2 * t4) + ocol0, yq1 = yoff(2 * t4 + 1 < n ? 2 * t4 + 1 : 0) + ocol0;
+    const long long yq8 = yoff(8 + 2 * t4 < n ? 8 + 2 * t4 : 0) + ocol0, yq9 = yoff(9 + 2 * t4 < n ? 9 + 2 * t4 : 0) + ocol0;
+    const long long xq_self = xoff(q);
+    const long long zrow = yoff(q) + ocol0;
+    const bool xph = HASPH && xwrap && ar.phd[0], yph = HASPH && ywrap && ar.phd[1];
+    const T WXq = sc.W[0][q], WYq = sc.W[1][q];
+    const T sXWY = sc.sdir[0] * WYq, sYWX = sc.sdir[1] * WXq;
+    // fragment-load offsets inside a plane stage (bytes, before the swizzle)
+    uint32_t xa[KS][KH], ya[KS][KH];
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+        for (int h = 0; h < KH; ++h) {
+            const int kk = kmap<MODE>(ks, h, t4) < n ? kmap<MODE>(ks, h, t4) : 0;
+            xa[ks][h] = (uint32_t)(q * n + kk) * 128u + fb0;
+            ya[ks][h] = (uint32_t)(kk * n + q) * 128u + fb0;
+        }
+    auto lds = [&](uint32_t lin) { return *reinterpret_cast<const T*>(smem + swz(lin)); };
 
     // conj(phase) on a wrapped output: own' = own pr + (ri ? -other pi : other pi), the partner component sits in lane ^ 4
     auto conj_phase = [&](T val, double pr, double pi) {
@@ -283,12 +333,11 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
         return (T)fma((double)other, ri ? -pi : pi, (double)val * pr);
     };
 
-    // ---- X task of plane tp: x-contraction of row q -> XR[tp & 1]
-    auto xtask = [&](int tp) {
-        T* IN = stage(tp);
+    // ---- X task of plane tp (ring slot base sb, R slot rsl): x-contraction of row q and S5 on its owned nodes -> XR[tp & 1]
+    auto xtask = [&](int tp, uint32_t sb, int rsl, int rpar, bool up, T inv_wz) {
         if (HASPH) {
-            // Bloch phase on wrapped entries of the landed plane (x: the face column; y: row P; z: the whole wrapped plane),
-            // fixed up in place before any task reads the plane (boundary CTAs only); this warp fixes row q of its spin
+            // Bloch phase on wrapped entries of the landed plane (x: node P of every line; y: line P; z: the whole wrapped
+            // plane), fixed up in place before any task reads the plane (boundary CTAs only); this warp fixes row q of its spin
             const bool wz = ar.phd[2] && (g0 + tp) == ar.n1[2];
             if (xph | yph | wz) {                                       // CTA-uniform
                 double br = 1.0, bi = 0.0;
@@ -301,12 +350,13 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                     double pr = br, pi = bi;
                     const bool fx = i == P && xph;
                     if (fx) { const double u = pr * ar.ph_re[0] - pi * ar.ph_im[0]; pi = pr * ar.ph_im[0] + pi * ar.ph_re[0]; pr = u; }
-                    T* e = IN + (i < P ? (q * P + i) * C : Cfg::FACE_ELEMS + q * C) + col0;
+                    const uint32_t lin = sb + (uint32_t)(q * n + (valid ? i : 0)) * 128u + fb0;
 #pragma unroll
                     for (int r = 0; r < NR; ++r) {
-                        const T val = valid ? e[8 * r] : (T)0;
+                        T* e = reinterpret_cast<T*>(smem + swz(lin + 8 * r * ESZ));
+                        const T val = valid ? *e : (T)0;
                         const T other = __shfl_xor_sync(0xffffffffu, val, 4);
-                        if (valid && (rowph || fx)) e[8 * r] = (T)fma((double)other, ri ? pi : -pi, (double)val * pr);
+                        if (valid && (rowph || fx)) *e = (T)fma((double)other, ri ? pi : -pi, (double)val * pr);
                     }
                 }
                 // these stage bytes are later rewritten by TMA.  No barrier here: this warp's X task reads only the row it
@@ -317,36 +367,57 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
         }
         Acc<P, MODE> acc;
         acc.zero();
-        const T* mainp = IN + (q * P) * C + col0;
-        const T* facep = IN + Cfg::FACE_ELEMS + q * C + col0;
-        contract<P, MODE, 0>(acc, bf, t4, [&](int, int, int kk, int r) { return kk < P ? mainp[kk * C + 8 * r] : facep[8 * r]; });
-        T* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / Cfg::ESZ) + (q * n) * XP + col0;
+        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, int r) { return lds(sb + xa[ks][h] + 8 * r * ESZ); });
+        T* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / ESZ) + (q * n) * XP + col0;
+        const bool s5on = up && q < P;
+        if (s5on) mbar_wait(&full_r[rsl], rpar);
+        const uint32_t rb = Cfg::R_OFF + (uint32_t)rsl * Cfg::R_STAGE;
+        const double* Fs = reinterpret_cast<const double*>(smem + rb + Cfg::R_BYTES) + (q * P) * 4;
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
+                if (nt * 8 + e >= n) continue;                           // nothing in this fragment column at all
                 const int xo = nt * 8 + 2 * t4 + e;
-                if (nt * 8 + 6 + e < n || xo < n) {
+                const bool live = nt * 8 + 6 + e < n || xo < n;          // compile-time true for fully populated n-tiles
+                const int xoc = live ? xo : 0;
+                double f0 = 0.0, f2 = 0.0, f3 = 0.0;
+                const bool own_node = s5on && live && (nt * 8 + 6 + e < P || xoc < P);
+                if (own_node) { f0 = Fs[xoc * 4 + mt]; f2 = Fs[xoc * 4 + 2]; f3 = sg * Fs[xoc * 4 + 3]; }
 #pragma unroll
-                    for (int r = 0; r < NR; ++r) XR[xo * XP + 8 * r] = WYq * acc.d[nt][r][e];
+                for (int r = 0; r < NR; ++r) {
+                    T val = sXWY * acc.d[nt][r][e];
+                    if (own_node) {
+                        // S5 on an owned node: eq. 12 spin blocks, in-term, R-term, divided by the plane's
+                        // z-weight because the Y task multiplies the whole XR entry by it
+                        const uint32_t lin = sb + (uint32_t)(q * n + xoc) * 128u + (fb0 & ~(uint32_t)(2 * ESZ - 1)) + 8 * r * ESZ;
+                        const T2 me = *reinterpret_cast<const T2*>(smem + swz(lin));
+                        const T2 ot = *reinterpret_cast<const T2*>(smem + swz(lin ^ 64u));
+                        const double own = ri ? (double)me.y : (double)me.x;
+                        const double osame = ri ? (double)ot.y : (double)ot.x, oflip = ri ? (double)ot.x : (double)ot.y;
+                        const double pot = fma(f0, own, fma(f2, osame, f3 * oflip));
+                        double s5 = fma(cin[r], own, sc.cHp * pot);
+                        if (ar.useR) {
+                            const uint32_t rl = rb + (uint32_t)((q * P + xoc) * C + col0 + 8 * r) * 8u;
+                            s5 = fma(cR[r], *reinterpret_cast<const double*>(smem + swz(rl)), s5);
+                        }
+                        val = fma((T)s5, inv_wz, val);
+                    }
+                    if (live) XR[xoc * XP + 8 * r] = val;
                 }
             }
+        if (up) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_r[rsl]);
+        }
     };
 
-    // ---- Y task of plane tp: y-contraction at x-position q, + XR, + S5 on owned nodes, RED to out (S3 + S5)
-    auto ytask = [&](int tp, int c, bool lower, bool upper) {
-        const T* IN = stage(tp);
-        const int rs = tp % RS;
-        const double* Rs = reinterpret_cast<const double*>(rring + (size_t)rs * Cfg::R_STAGE);
-        const double* Fs = reinterpret_cast<const double*>(rring + (size_t)rs * Cfg::R_STAGE + Cfg::R_BYTES);
+    // ---- Y task of plane tp: y-contraction at x-position q, + XR (x part and S5), times the plane's z-weight -> RED to out
+    auto ytask = [&](int tp, uint32_t sb, T wz) {
         Acc<P, MODE> acc;
         acc.zero();
-        const T* base = IN + (q < P ? q * C : Cfg::FACE_ELEMS) + col0;
-        const int stride = q < P ? P * C : C;
-        contract<P, MODE, 1>(acc, bf, t4, [&](int, int, int kk, int r) { return base[kk * stride + 8 * r]; });
-        const T* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / Cfg::ESZ) + q * XP + col0;
-        // the plane's in-plane part belongs to the cell above (weight W_z[c]) and, on a cell boundary, to the cell below (W_z[P])
-        const T wz = (upper ? sc.W[2][c] : (T)0) + (lower ? sc.W[2][P] : (T)0);
+        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, int r) { return lds(sb + ya[ks][h] + 8 * r * ESZ); });
+        const T* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / ESZ) + q * XP + col0;
         const bool zwrap = (g0 + tp) == ar.n1[2];
         const bool zp = HASPH && zwrap && ar.phd[2];
         const bool anyph = HASPH && ((q == P && xph) || yph || zp);    // warp-uniform
@@ -357,61 +428,49 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
             pr1 = pr0; pi1 = pi0;
             if (yph) { pr1 = pr0 * ar.ph_re[1] - pi0 * ar.ph_im[1]; pi1 = pr0 * ar.ph_im[1] + pi0 * ar.ph_re[1]; }
         }
-        if (upper && q < P) mbar_wait(&full_r[rs], (tp / RS) & 1);
-        T* const pbase = outp + zoff(g0 + tp) + xoff(q);
+        T* const pbase = outp + zoff(g0 + tp) + xq_self;
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
+                if (nt * 8 + e >= n) continue;
                 const int yo = nt * 8 + 2 * t4 + e;
-                const bool live = nt * 8 + 6 + e < n || yo < n;          // compile-time true for fully populated n-tiles
-                if (nt * 8 + e >= n) continue;                           // nothing in this fragment column at all
+                const bool live = nt * 8 + 6 + e < n || yo < n;
                 const int yoc = live ? yo : 0;
-                const long long yo_off = yoff(yoc);
+                const long long yq = nt == 0 ? (e == 0 ? yq0 : yq1) : (e == 0 ? yq8 : yq9);
 #pragma unroll
                 for (int r = 0; r < NR; ++r) {
-                    T val = wz * fma(WXq, acc.d[nt][r][e], XR[(yoc * n) * XP + 8 * r]);
-                    if (upper && q < P && live && yoc < P) {
-                        // S5 on an owned node: eq. 12 spin blocks, in-term, R-term
-                        const int o = (yoc * P + q) * C + col0 + 8 * r;
-                        const double own = (double)IN[o];
-                        const double osame = (double)IN[o + ((col0 ^ MROWS) - col0)];
-                        const double oflip = (double)IN[o + ((col0 ^ MROWS ^ 1) - col0)];
-                        const double* f = Fs + (yoc * P + q) * 4;
-                        const double pot = fma(f[mt], own, fma(f[2], osame, (sg * f[3]) * oflip));
-                        double s5 = fma(cin[r], own, sc.cHp * pot);
-                        if (ar.useR) s5 = fma(cR[r], Rs[o], s5);
-                        val += (T)s5;
-                    }
+                    T val = wz * fma(sYWX, acc.d[nt][r][e], XR[(yoc * n) * XP + 8 * r]);
                     if (anyph) val = conj_phase(val, yoc == P ? pr1 : pr0, yoc == P ? pi1 : pi0);
-                    if (live && vok[r]) red_add_t(pbase + yo_off + ocol[r], val);
+                    if (live && vok[r]) red_add_t(pbase + yq + 8 * r, val);
                 }
             }
-        if (upper) {
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_r[rs]);
-        }
     };
 
-    // ---- Z task of the cell whose planes are tb .. tb + P: z-contraction for the nodes of row q, RED to out
-    auto ztask = [&](int tb) {
-        // this lane's planes kk = t4 + 4 h (+ KSTEP ks): element pointers into the ring
-        const T* pl[Cfg::KS][Cfg::KH];
+    // ---- Z task of the cell whose planes sit in ring slots sl0, sl0+1, ... (mod S), first plane tb: z-contraction for the
+    //      nodes of row q -> RED to out
+    auto ztask = [&](int tb, int sl0) {
+        uint32_t zb[KS][KH];                       // this lane's planes: stage base + the row's first node
 #pragma unroll
-        for (int ks = 0; ks < Cfg::KS; ++ks)
+        for (int ks = 0; ks < KS; ++ks)
 #pragma unroll
-            for (int h = 0; h < Cfg::KH; ++h) {
-                const int kk = ks * Cfg::KSTEP + t4 + 4 * h;
-                pl[ks][h] = stage(tb + (kk < n ? kk : 0)) + col0;
+            for (int h = 0; h < KH; ++h) {
+                const int kk = kmap<MODE>(ks, h, t4) < n ? kmap<MODE>(ks, h, t4) : 0;
+                int sl = sl0 + kk; if (sl >= S) sl -= S;
+                zb[ks][h] = (uint32_t)sl * Cfg::IN_STAGE + (uint32_t)(q * n) * 128u + fb0;
             }
         const bool zwrap = (g0 + tb + P) == ar.n1[2];
         const bool zp = HASPH && zwrap && ar.phd[2];
-        T* const rowbase = outp + yoff(q);
+        // this thread's output planes: tb + 2 t4 + e, and tb + 8 + 2 t4 + e (live only where < n)
+        const long long zq0 = zoff(g0 + tb + 2 * t4) + zrow, zq1 = zoff(g0 + tb + (2 * t4 + 1 < n ? 2 * t4 + 1 : 0)) + zrow;
+        const long long zq8 = zoff(g0 + tb + (8 + 2 * t4 < n ? 8 + 2 * t4 : 0)) + zrow;
+        const long long zq9 = zoff(g0 + tb + (9 + 2 * t4 < n ? 9 + 2 * t4 : 0)) + zrow;
+#pragma unroll 1
         for (int i = 0; i < n; ++i) {
-            const int noff = i < P ? (q * P + i) * C : Cfg::FACE_ELEMS + q * C;
             Acc<P, MODE> acc;
             acc.zero();
-            contract<P, MODE, 2>(acc, bf, t4, [&](int ks, int h, int, int r) { return pl[ks][h][noff + 8 * r]; });
+            const uint32_t no = (uint32_t)i * 128u;
+            contract<P, MODE>(acc, bf, t4, [&](int ks, int h, int r) { return lds(zb[ks][h] + no + 8 * r * ESZ); });
             const T w = sc.W[0][i] * WYq;
             const bool anyph = HASPH && ((i == P && xph) || (q == P && yph) || zp);
             double pr0 = 1.0, pi0 = 0.0, pr1 = 1.0, pi1 = 0.0;          // conj phase of planes < P / of the wrapped top plane
@@ -421,79 +480,107 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 pr1 = pr0; pi1 = pi0;
                 if (zp) { pr1 = pr0 * ar.ph_re[2] - pi0 * ar.ph_im[2]; pi1 = pr0 * ar.ph_im[2] + pi0 * ar.ph_re[2]; }
             }
-            T* const nb = rowbase + xoff(i);
+            T* const nb = outp + xoff(i);
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
+                    if (nt * 8 + e >= n) continue;
                     const int ko = nt * 8 + 2 * t4 + e;
                     const bool live = nt * 8 + 6 + e < n || ko < n;
-                    if (nt * 8 + e >= n) continue;
                     const int koc = live ? ko : 0;
-                    const long long zo = zoff(g0 + tb + koc);
+                    const long long zq = nt == 0 ? (e == 0 ? zq0 : zq1) : (e == 0 ? zq8 : zq9);
 #pragma unroll
                     for (int r = 0; r < NR; ++r) {
                         T val = w * acc.d[nt][r][e];
                         if (anyph) val = conj_phase(val, koc == P ? pr1 : pr0, koc == P ? pi1 : pi0);
-                        if (live && vok[r]) red_add_t(nb + zo + ocol[r], val);
+                        if (live && vok[r]) red_add_t(nb + zq + 8 * r, val);
                     }
                 }
         }
     };
 
-    // ---- march
+    // ---- march.  Plane t sits in ring slot t mod S (sl), its R / fields in slot t mod RS; c = t mod P is its index in the
+    //      cell above it.  In-plane weight of plane t: W_z[c] for the cell above (if any) + W_z[P] for the cell below (if any).
+    auto zweight = [&](int t, int c) {
+        return (t < T_ - 1 ? sc.W[2][c] : (T)0) + ((c == 0 && t > 0) ? sc.W[2][P] : (T)0);
+    };
     mbar_wait(&full_in[0], 0);
-    xtask(0);
+    xtask(0, 0u, 0, 0, true, (T)1 / zweight(0, 0));
     asm volatile("bar.sync 1, %0;" ::"r"(NTH) : "memory");
-    int c = 0;
+    int c = 0, sl = 0, par = 0;                    // of plane t
+    int rsl = 1 % RS, rpar = (1 / RS) & 1;         // R slot / parity of plane t + 1
+    int cell_sl = 0;                               // ring slot of the first plane of the cell being filled
 #pragma unroll 1
     for (int t = 0; t < T_; ++t) {
         const bool lower = c == 0 && t > 0, upper = t < T_ - 1;
+        int sl1 = sl + 1, par1 = par; if (sl1 == S) { sl1 = 0; par1 ^= 1; }
+        const int c1 = (c + 1 == P) ? 0 : c + 1;
         if (upper) {
-            mbar_wait(&full_in[(t + 1) % S], ((t + 1) / S) & 1);
-            xtask(t + 1);                         // XR[(t+1)&1] was last read in the Y task of plane t-1, before the last barrier
+            mbar_wait(&full_in[sl1], par1);
+            // XR[(t+1)&1] was last read in the Y task of plane t-1, before the last barrier
+            xtask(t + 1, (uint32_t)sl1 * Cfg::IN_STAGE, rsl, rpar, t + 1 < T_ - 1, (T)1 / zweight(t + 1, c1));
+            if (++rsl == RS) { rsl = 0; rpar ^= 1; }
         }
-        ytask(t, c, lower, upper);
+        ytask(t, (uint32_t)sl * Cfg::IN_STAGE, zweight(t, c));
         if (lower) {
-            ztask(t - P);                         // the cell below is complete and all its planes are still resident
+            ztask(t - P, cell_sl);                 // the cell below is complete and all its planes are still resident
             __syncwarp();
-            if (lane == 0)
-                for (int k = t - P; k < t; ++k) mbar_arrive(&empty_in[k % S]);     // its planes but the shared top one
+            if (lane == 0) {
+                int k = cell_sl;
+                for (int j = 0; j < P; ++j) { mbar_arrive(&empty_in[k]); if (++k == S) k = 0; }   // its planes but the shared top one
+            }
+            cell_sl = sl;
         }
         asm volatile("bar.sync 1, %0;" ::"r"(NTH) : "memory");
-        c = (c + 1 == P) ? 0 : c + 1;
+        c = c1; sl = sl1; par = par1;
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // All scalings (1/2, Jacobian, D^-1 on the way in, M^-1 on the way out, the step coefficient) folded into the 1-D tables.
+// On this mesh the three scaled 1-D operators are one matrix times a scalar per direction (the directions differ only in
+// h_d): the kernel keeps the z-direction matrix and the two ratios.
 template <typename T>
-static void build_mma_const(const chfsi_mesh* m, const CellArgs& a, MmaConst<T>& sc) {
+static bool build_mma_const(const chfsi_mesh* m, const CellArgs& a, MmaConst<T>& sc) {
     const MeshConst& mc = m->mc;
     const int n = mc.n;
     const bool sin_ = (a.flags & kScaleIn) != 0, sout_ = (a.flags & kSoutInvM) != 0;
     std::memset(&sc, 0, sizeof(sc));
     sc.cHp = a.cH;
+    double K[3][kMaxN][kMaxN];
     for (int d = 0; d < 3; ++d)
         for (int i = 0; i < n; ++i) {
             const double si = sin_ ? mc.im1[d][i] : 1.0, so = sout_ ? mc.im1[d][i] : 1.0;
             for (int b = 0; b < n; ++b) {
                 const double sb = sin_ ? mc.im1[d][b] : 1.0;
                 // the step coefficient rides on the x-direction factors: on K_x for the x part and on W_x for the y and z parts
-                sc.K[d][i][b] = (T)((d == 0 ? a.cH : 1.0) * so * mc.Kd[d][i][b] * sb);
+                K[d][i][b] = (d == 0 ? a.cH : 1.0) * so * mc.Kd[d][i][b] * sb;
             }
             sc.W[d][i] = (T)((d == 0 ? a.cH : 1.0) * mc.w[i] * so * si);
         }
+    if (K[2][0][0] == 0.0) return false;
+    double amax = 0.0;
+    for (int i = 0; i < n; ++i)
+        for (int b = 0; b < n; ++b) { sc.K[i][b] = (T)K[2][i][b]; amax = std::fmax(amax, std::fabs(K[2][i][b])); }
+    for (int d = 0; d < 3; ++d) {
+        const double s = K[d][0][0] / K[2][0][0];
+        for (int i = 0; i < n; ++i)
+            for (int b = 0; b < n; ++b)
+                if (std::fabs(K[d][i][b] - s * K[2][i][b]) > 1e-12 * std::fabs(s) * amax) return false;   // not proportional
+        sc.sdir[d] = (T)s;
+    }
+    return true;
 }
 
-static std::once_flag g_mma_attr_once[4][3][2][32];   // [p/2 - 1][mode][phase][device]
+static std::once_flag g_mma_attr_once[4][3][4][32];   // [p/2 - 1][mode][phase, full tiles][device]
 
 template <int P, int MODE>
 static cudaError_t launch_mma_t(const chfsi_mesh* m, const CellArgs& a, cudaStream_t st) {
     using Cfg = MmaCfg<P, MODE>;
     using T = typename Cfg::T;
     MmaConst<T> sc;
-    build_mma_const<T>(m, a, sc);
+    if (!build_mma_const<T>(m, a, sc)) return cudaErrorInvalidValue;
     MarchArgs ar;
     std::memset(&ar, 0, sizeof(ar));
     for (int d = 0; d < 3; ++d) {
@@ -514,18 +601,23 @@ static cudaError_t launch_mma_t(const chfsi_mesh* m, const CellArgs& a, cudaStre
     constexpr int BC = Cfg::C / 2;
     constexpr bool f32 = sizeof(T) == 4;
     const int nl[3] = {P + 1, P, 1};
+    // with a single cell in x the 2(P+1)-row box would not fit the x-line: such meshes always take the per-line path
+    const int rows_full = ar.nc[0] > 1 ? 2 * (P + 1) : 2 * P;
     for (int i = 0; i < 3; ++i)
-        if (!make_map3(&mp.main[i], m, a.in, a.ld_in, a.nvec, BC, 2 * P, nl[i], f32) ||
-            !make_map3(&mp.face[i], m, a.in, a.ld_in, a.nvec, BC, 2, nl[i], f32))
-            return cudaErrorInvalidValue;
-    if (!make_map3(&mp.R, m, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, a.nvec, BC, 2 * P, P, ar.useR ? false : f32) ||
+        if (!make_map3(&mp.main[i], m, a.in, a.ld_in, a.nvec, BC, rows_full, nl[i], f32, kSwizzle)) return cudaErrorInvalidValue;
+    if (!make_map3(&mp.face[0], m, a.in, a.ld_in, a.nvec, BC, 2 * P, 1, f32, kSwizzle) ||
+        !make_map3(&mp.face[1], m, a.in, a.ld_in, a.nvec, BC, 2, 1, f32, kSwizzle) ||
+        !make_map3(&mp.face[2], m, a.in, a.ld_in, a.nvec, BC, 2, 1, f32, kSwizzle))
+        return cudaErrorInvalidValue;
+    if (!make_map3(&mp.R, m, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, a.nvec, BC, 2 * P, P, ar.useR ? false : f32, kSwizzle) ||
         !make_mapF(&mp.F, m, P))
         return cudaErrorInvalidValue;
     if (a.flags & kMassIn) return cudaErrorInvalidValue;             // the residual S0 runs on the line-owned FP64 kernel
-    const bool ph = m->mc.has_phase != 0;
-    auto kern = ph ? cell_mma_kernel<P, MODE, true> : cell_mma_kernel<P, MODE, false>;
+    const bool ph = m->mc.has_phase != 0, full = a.nvec % Cfg::NV == 0;
+    auto kern = ph ? (full ? cell_mma_kernel<P, MODE, true, true> : cell_mma_kernel<P, MODE, true, false>)
+                   : (full ? cell_mma_kernel<P, MODE, false, true> : cell_mma_kernel<P, MODE, false, false>);
     cudaError_t attr_err = cudaSuccess;
-    std::call_once(g_mma_attr_once[P / 2 - 1][MODE][ph ? 1 : 0][m->device & 31], [&] {
+    std::call_once(g_mma_attr_once[P / 2 - 1][MODE][(ph ? 2 : 0) + (full ? 1 : 0)][m->device & 31], [&] {
         attr_err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
     });
     if (attr_err != cudaSuccess) return attr_err;
