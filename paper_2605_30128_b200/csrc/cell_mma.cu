@@ -19,11 +19,15 @@
 //   Y task (warp = x-position i):  y-contraction at x-position i of plane t, + XR             -> RED to `out`
 //   Z task (at the end of a cell): z-contraction over the p+1 planes of the cell, which are all resident in the plane
 //                                  ring (no z accumulators in registers), for the warp's row of nodes -> RED to `out`
-// D comes out as (column g, outputs 2t, 2t+1): eight lanes hold eight adjacent columns, so every RED covers full 32-byte
-// sectors.  An output node receives two REDs (in-plane part + S5, z part) instead of one.
-// Shared-memory layout: a plane is [p+1 lines][p+1 nodes][128 B] (the x = P face column sits inline as node P of its line),
-// landed by TMA with the 128-byte swizzle; fragment loads whose four k-lanes differ in node, line or plane then hit
-// distinct banks (the plane pitch is 2 mod 8 rows of 128 B, the ring has a multiple of 4 slots, k is interleaved 2t, 2t+1).
+// Fragment rows are chosen so that a thread's 8-byte unit of a node's 128-byte row -- one complex64 (TF32: rows g and g+8 of
+// the m16 tile are its real and imaginary part) or one double (FP64) -- is: bit 3 = g & 1, bit 6 (the spin component) =
+// (g >> 1) & 1, the 16-byte chunk = 2 mt + (g >> 2).  A half-warp then reads 16 distinct 8-byte slots of every landed row,
+// D comes out as complex values per thread (TF32: one red.global.add.v2.f32 per output), and the lanes of a RED cover
+// full 32-byte sectors.  An output node receives two REDs (in-plane part + S5, z part) instead of one.
+// Shared-memory layout: a plane is [p+1 lines][p+1 nodes][2 spins][64 B] (the x = P face column sits inline as node P of its
+// line), landed by TMA with the 64-byte swizzle (16-byte chunk index ^= 128-byte row index mod 4): the four k-lanes of a
+// fragment load differ in node, line or plane, i.e. in the row index mod 4 (rows per line and per plane are odd, the ring has
+// a multiple of 4 slots), so every fragment load is bank-conflict free.
 // Modes: MM_F64 (complex128 storage, mma.m8n8k4.f64), MM_TF32 (complex64 storage, operands rounded to TF32 by
 // round-to-nearest-away, FP32 accumulate: CHFSI_TF32), MM_TF32X3 (hi/lo split of both operands, three MMAs, small terms
 // first: CHFSI_TF32X3).
@@ -52,7 +56,7 @@ struct MmaConst {
     double cHp;                 // coefficient of the potential term
 };
 
-constexpr bool kSwizzle = false; // 128-byte TMA swizzle of the plane and R stages (false: linear layout, for debugging)
+constexpr bool kSwizzle = true;  // TMA swizzle of the plane and R stages (false: linear layout, for debugging)
 
 template <int P, int MODE>
 struct MmaCfg {
@@ -66,17 +70,18 @@ struct MmaCfg {
     static constexpr int THREADS = (NCW + 1) * 32;
     static constexpr int ESZ = (int)sizeof(T);
     static_assert(C * ESZ == 128, "one node of the CTA's columns is one 128-byte row");
-    // plane ring stage: [n lines][n nodes][128 B]; pitch = n^2 + 1 rows of 128 B (n odd => n^2 = 1 mod 8 => pitch = 2 mod 8)
+    // plane ring stage: [n lines][n nodes][128 B]; n is odd, so a line and a plane are an odd number of 128-byte rows
     static constexpr int LINE_BYTES = n * 128;
     static constexpr int IN_BYTES = n * n * 128;
-    static constexpr int IN_STAGE = (n * n + 1) * 128;
+    static constexpr int IN_STAGE = IN_BYTES;
+    static_assert(n % 2 == 1, "even degrees only");
     // R / fields ring stage: R [P lines][P nodes][2 spins][C/2 doubles] | fields [P][P][4] f64
     static constexpr int R_BYTES = P * P * C * 8, F_BYTES = P * P * 32;
     static constexpr int R_STAGE = ((R_BYTES + F_BYTES + 1023) / 1024) * 1024;
     static constexpr int RS = 3;
-    // XR[row][x'][XP]: the x-contraction of a plane, column pitch padded by 16 bytes (bank spread of the fragment accesses)
-    static constexpr int XP = C + 16 / ESZ;
-    static constexpr int XR_BYTES = ((n * n * XP * ESZ + 127) / 128) * 128;
+    // XR[row][x'][XPU units of 8 bytes]: the x-contraction of a plane; 16 units per node + 1 of padding (bank spread)
+    static constexpr int XPU = 17;
+    static constexpr int XR_BYTES = ((n * n * XPU * 8 + 127) / 128) * 128;
     static constexpr int S_ = ((219 * 1024 - 2 * XR_BYTES - RS * R_STAGE) / IN_STAGE) / 4 * 4;     // a multiple of 4 slots
     static constexpr int S = S_ < 16 ? S_ : 16;
     static_assert(S >= P + 2, "plane ring must hold a whole cell plus the plane ahead");
@@ -85,12 +90,17 @@ struct MmaCfg {
     static constexpr size_t SMEM = (size_t)XR_OFF + 2 * (size_t)XR_BYTES + 1024;   // + slack to align the base to 1024 B
 };
 
-// byte offset (from the 1024-aligned base) -> swizzled byte offset: the 16-byte chunk index (bits 4..6) is XORed with the
-// 128-byte row index (bits 7..9), which is what CU_TENSOR_MAP_SWIZZLE_128B does to the bytes TMA writes
-__device__ __forceinline__ uint32_t swz(uint32_t lin) { return kSwizzle ? lin ^ ((lin >> 3) & 0x70u) : lin; }
+// byte offset (from the 1024-aligned base) -> swizzled byte offset, as TMA lays the bytes out (measured on the B200 with a
+// probe kernel: the pattern is a function of the absolute shared-memory address):
+//   CU_TENSOR_MAP_SWIZZLE_64B : 16-byte chunk index bits 4..5 ^= 128-byte row index bits 7..8, rows of 64 bytes stay dense
+//   CU_TENSOR_MAP_SWIZZLE_128B: chunk index bits 4..6 ^= row index bits 7..9 (used where the box rows are 128 bytes)
+__device__ __forceinline__ uint32_t swz64(uint32_t lin) { return kSwizzle ? lin ^ ((lin >> 3) & 0x30u) : lin; }
+__device__ __forceinline__ uint32_t swz128(uint32_t lin) { return kSwizzle ? lin ^ ((lin >> 3) & 0x70u) : lin; }
 
 __device__ __forceinline__ void red_add_t(double* p, double v) { atomicAdd(p, v); }     // result unused -> RED
-__device__ __forceinline__ void red_add_t(float* p, float v) { atomicAdd(p, v); }
+__device__ __forceinline__ void red_add_c64(float* p, float re, float im) {             // one complex64: 8-byte vector RED
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(re), "f"(im) : "memory");
+}
 
 // round-to-nearest, ties away from zero, to the 10-bit TF32 mantissa (what cvt.rna.tf32.f32 returns for finite inputs):
 // add half an ulp of TF32 to the magnitude bits; the tensor core ignores the low 13 bits
@@ -108,12 +118,11 @@ __device__ __forceinline__ void mma_f64(double (&d)[1][2], double a, double b) {
                  : "+d"(d[0][0]), "+d"(d[0][1]) : "d"(a), "d"(b));
 }
 
-// The line index that fragment position (k-step ks, half h, lane t) contracts over.  TF32: k = t and k = t + 4 of a k-step are
-// mapped to the neighbouring nodes 2t and 2t+1, so that the four lanes of a load differ in bits 1..2 of the 128-byte row
-// index and the swizzle spreads them over all banks.  Any permutation is legal as long as A and B use the same one.
+// The line index that fragment position (k-step ks, half h, lane t) contracts over: the four lanes of a load read four
+// consecutive nodes / lines / planes, whose 128-byte row indices differ mod 4.
 template <int MODE>
 __device__ __forceinline__ int kmap(int ks, int h, int t) {
-    return MODE == MM_F64 ? ks * 4 + t : ks * 8 + 2 * t + h;
+    return MODE == MM_F64 ? ks * 4 + t : ks * 8 + t + 4 * h;
 }
 
 // B fragments of the base 1-D operator, per thread: B[k = in][n = out] = K[out][in]
@@ -158,7 +167,8 @@ struct Acc {
     }
 };
 
-// acc += K applied along the line whose element kmap(ks, h, t) for fragment row r is ld(ks, h, r)
+// acc += K applied along the line whose 8-byte unit at element kmap(ks, h, t) is ld(ks, h): a double (FP64, fragment row g)
+// or a float2 = (fragment row g, fragment row g + 8) (TF32)
 template <int P, int MODE, typename LD>
 __device__ __forceinline__ void contract(Acc<P, MODE>& acc, const BFrags<P, MODE>& bf, int t, LD ld) {
     using Cfg = MmaCfg<P, MODE>;
@@ -171,8 +181,12 @@ __device__ __forceinline__ void contract(Acc<P, MODE>& acc, const BFrags<P, MODE
             // the last k-step is only partly populated: lanes beyond the line contribute zeros
             const bool all = kmap<MODE>(ks, h, 3) < Cfg::n;
             const bool ok = all || kmap<MODE>(ks, h, t) < Cfg::n;
-#pragma unroll
-            for (int r = 0; r < Cfg::NR; ++r) a[r][h] = ok ? ld(ks, h, r) : (T)0;
+            if constexpr (MODE == MM_F64) {
+                a[0][h] = ok ? ld(ks, h) : 0.0;
+            } else {
+                const float2 u = ok ? ld(ks, h) : make_float2(0.f, 0.f);
+                a[0][h] = u.x; a[1][h] = u.y;
+            }
         }
         if constexpr (MODE == MM_F64) {
 #pragma unroll
@@ -204,14 +218,15 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 const __grid_constant__ MarchMaps mp) {
     using Cfg = MmaCfg<P, MODE>;
     using T = typename Cfg::T;
-    using T2 = typename std::conditional<MODE == MM_F64, double2, float2>::type;
-    constexpr int n = Cfg::n, C = Cfg::C, S = Cfg::S, RS = Cfg::RS, XP = Cfg::XP, NR = Cfg::NR, NT = Cfg::NT, MROWS = Cfg::MROWS;
+    constexpr bool F64 = MODE == MM_F64;
+    using U = typename std::conditional<F64, double, float2>::type;      // the thread's 8-byte unit of a node row
+    constexpr int n = Cfg::n, C = Cfg::C, S = Cfg::S, RS = Cfg::RS, XPU = Cfg::XPU, NR = Cfg::NR, NT = Cfg::NT;
     constexpr int ESZ = Cfg::ESZ, KS = Cfg::KS, KH = Cfg::KH;
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t full_in[S], empty_in[S], full_r[RS], empty_r[RS];
-    // the swizzle is a function of shared-memory address bits 4..9: work from a 1024-byte aligned base
+    // the swizzle is a function of shared-memory address bits: work from a 1024-byte aligned base
     unsigned char* const smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    T* const XRb = reinterpret_cast<T*>(smem + Cfg::XR_OFF);
+    U* const XRb = reinterpret_cast<U*>(smem + Cfg::XR_OFF);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     constexpr int ROWB = (C / 2) * ESZ;
@@ -280,29 +295,27 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
     }
 
     // ================================ consumers ================================
-    const int mt = warp & 1, q = warp >> 1;       // spin component (= m-tile); index: row j (X, Z tasks) / x-position i (Y task)
+    // warp = (index q in 0..p: row j of the X and Z tasks, x-position i of the Y task) x (m-tile mt: half of the CTA's vectors)
+    const int mt = warp & 1, q = warp >> 1;
     const int g = lane >> 2, t4 = lane & 3;
-    const int col0 = mt * MROWS + g;              // fragment row r is column col0 + 8 r
-    const uint32_t fb0 = (uint32_t)col0 * ESZ;    // its byte offset inside a node's 128-byte row
-    const int ri = g & 1;
-    const double sg = ((ri == 0) != (mt == 0)) ? -1.0 : 1.0;
+    // the thread's 8-byte unit inside a node's 128-byte row: bit 3 = g & 1, spin (bit 6) = (g >> 1) & 1, chunk = 2 mt + (g >> 2)
+    const int spin = (g >> 1) & 1;
+    const uint32_t fb0 = (uint32_t)(spin * 64 + (2 * mt + (g >> 2)) * 16 + (g & 1) * 8);
+    const int upos = (int)(fb0 >> 3);             // unit index inside the node (XR)
+    // TF32: unit = complex64 of vector vl; FP64: unit = the re (ri = 0) or im (ri = 1) part of vector vl
+    const int vl = F64 ? 2 * mt + (g >> 2) : 4 * mt + 2 * (g >> 2) + (g & 1);
+    const int ri = F64 ? (g & 1) : 0;
+    const double sgs = spin == 0 ? 1.0 : -1.0;    // sign of B_y in (B_x -+ i B_y)
     const int NTH = Cfg::NCW * 32;
     BFrags<P, MODE> bf;
     bf.init(sc, g, t4);
-    bool vok[NR];
-    double cin[NR], cR[NR];
-    int v0 = 0;
-#pragma unroll
-    for (int r = 0; r < NR; ++r) {
-        const int v = chunk * Cfg::NV + ((8 * r + g) >> 1);
-        vok[r] = FULLV || v < ar.nvec;
-        if (r == 0) v0 = v;
-        cin[r] = (vok[r] && ar.cin) ? __ldg(ar.cin + v) : 0.0;
-        cR[r] = (vok[r] && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
-    }
-    // `out` offsets in scalars of T: node I -> 4 ld I; spin -> 2 ld; vector v -> 2 v; fragment row r = 1 is 4 vectors on
+    const int v = chunk * Cfg::NV + vl;
+    const bool vok = FULLV || v < ar.nvec;
+    const double cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
+    const double cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
+    // `out` offsets in scalars of T: node I -> 4 ld I; spin -> 2 ld; vector v -> 2 v (+ ri)
     const long long XS = 4 * ar.ld_out, LS = (long long)ar.n1[0] * XS, PS = (long long)ar.n1[1] * LS;
-    const long long ocol0 = ((long long)mt * ar.ld_out + (FULLV || v0 < ar.nvec ? v0 : 0)) * 2 + ri;
+    const long long ocol0 = ((long long)spin * ar.ld_out + (vok ? v : 0)) * 2 + ri;
     T* const outp = reinterpret_cast<T*>(ar.out);
     auto xoff = [&](int i) { int gx = ex * P + i; if (gx == ar.n1[0]) gx = 0; return (long long)gx * XS; };
     auto yoff = [&](int j) { int gy = ey * P + j; if (gy == ar.n1[1]) gy = 0; return (long long)gy * LS; };
@@ -325,19 +338,31 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
             xa[ks][h] = (uint32_t)(q * n + kk) * 128u + fb0;
             ya[ks][h] = (uint32_t)(kk * n + q) * 128u + fb0;
         }
-    auto lds = [&](uint32_t lin) { return *reinterpret_cast<const T*>(smem + swz(lin)); };
+    auto ldu = [&](uint32_t lin) { return *reinterpret_cast<const U*>(smem + swz64(lin)); };
 
-    // conj(phase) on a wrapped output: own' = own pr + (ri ? -other pi : other pi), the partner component sits in lane ^ 4
-    auto conj_phase = [&](T val, double pr, double pi) {
-        const T other = __shfl_xor_sync(0xffffffffu, val, 4);
-        return (T)fma((double)other, ri ? -pi : pi, (double)val * pr);
+    // a complex output value held as d[0] = re, d[1] = im (TF32) or as the component ri of it (FP64, partner in lane ^ 4)
+    struct Val { T a, b; };
+    // multiply by conj(phase) = pr - i pi
+    auto conj_phase = [&](Val x, double pr, double pi) {
+        if constexpr (F64) {
+            const double other = __shfl_xor_sync(0xffffffffu, x.a, 4);
+            x.a = fma(other, ri ? -pi : pi, x.a * pr);                   // re' = re pr + im pi ; im' = im pr - re pi
+        } else {
+            const float re = (float)fma((double)x.b, pi, (double)x.a * pr), im = (float)fma((double)x.a, -pi, (double)x.b * pr);
+            x.a = re; x.b = im;
+        }
+        return x;
+    };
+    auto emit = [&](T* p, Val x) {
+        if constexpr (F64) red_add_t(p, x.a);
+        else red_add_c64(p, x.a, x.b);
     };
 
     // ---- X task of plane tp (ring slot base sb, R slot rsl): x-contraction of row q and S5 on its owned nodes -> XR[tp & 1]
     auto xtask = [&](int tp, uint32_t sb, int rsl, int rpar, bool up, T inv_wz) {
         if (HASPH) {
             // Bloch phase on wrapped entries of the landed plane (x: node P of every line; y: line P; z: the whole wrapped
-            // plane), fixed up in place before any task reads the plane (boundary CTAs only); this warp fixes row q of its spin
+            // plane), fixed up in place before any task reads the plane (boundary CTAs only); this warp fixes row q of its units
             const bool wz = ar.phd[2] && (g0 + tp) == ar.n1[2];
             if (xph | yph | wz) {                                       // CTA-uniform
                 double br = 1.0, bi = 0.0;
@@ -350,16 +375,19 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                     double pr = br, pi = bi;
                     const bool fx = i == P && xph;
                     if (fx) { const double u = pr * ar.ph_re[0] - pi * ar.ph_im[0]; pi = pr * ar.ph_im[0] + pi * ar.ph_re[0]; pr = u; }
-                    const uint32_t lin = sb + (uint32_t)(q * n + (valid ? i : 0)) * 128u + fb0;
-#pragma unroll
-                    for (int r = 0; r < NR; ++r) {
-                        T* e = reinterpret_cast<T*>(smem + swz(lin + 8 * r * ESZ));
-                        const T val = valid ? *e : (T)0;
-                        const T other = __shfl_xor_sync(0xffffffffu, val, 4);
-                        if (valid && (rowph || fx)) *e = (T)fma((double)other, ri ? pi : -pi, (double)val * pr);
+                    U* e = reinterpret_cast<U*>(smem + swz64(sb + (uint32_t)(q * n + (valid ? i : 0)) * 128u + fb0));
+                    if constexpr (F64) {
+                        const double val = valid ? *e : 0.0;
+                        const double other = __shfl_xor_sync(0xffffffffu, val, 4);
+                        if (valid && (rowph || fx)) *e = fma(other, ri ? pi : -pi, val * pr);   // re' = re pr - im pi ; im' = im pr + re pi
+                    } else {
+                        if (valid && (rowph || fx)) {
+                            const float2 z = *e;
+                            *e = make_float2((float)fma((double)z.y, -pi, (double)z.x * pr), (float)fma((double)z.x, pi, (double)z.y * pr));
+                        }
                     }
                 }
-                // these stage bytes are later rewritten by TMA.  No barrier here: this warp's X task reads only the row it
+                // these stage bytes are later rewritten by TMA.  No barrier here: this warp's X task reads only the units it
                 // fixed; every other reader of the plane (Y and Z tasks) runs after the barrier that ends the step.
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
@@ -367,8 +395,8 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
         }
         Acc<P, MODE> acc;
         acc.zero();
-        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, int r) { return lds(sb + xa[ks][h] + 8 * r * ESZ); });
-        T* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / ESZ) + (q * n) * XP + col0;
+        contract<P, MODE>(acc, bf, t4, [&](int ks, int h) { return ldu(sb + xa[ks][h]); });
+        U* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / 8) + (q * n) * XPU + upos;
         const bool s5on = up && q < P;
         if (s5on) mbar_wait(&full_r[rsl], rpar);
         const uint32_t rb = Cfg::R_OFF + (uint32_t)rsl * Cfg::R_STAGE;
@@ -381,29 +409,41 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 const int xo = nt * 8 + 2 * t4 + e;
                 const bool live = nt * 8 + 6 + e < n || xo < n;          // compile-time true for fully populated n-tiles
                 const int xoc = live ? xo : 0;
-                double f0 = 0.0, f2 = 0.0, f3 = 0.0;
                 const bool own_node = s5on && live && (nt * 8 + 6 + e < P || xoc < P);
-                if (own_node) { f0 = Fs[xoc * 4 + mt]; f2 = Fs[xoc * 4 + 2]; f3 = sg * Fs[xoc * 4 + 3]; }
-#pragma unroll
-                for (int r = 0; r < NR; ++r) {
-                    T val = sXWY * acc.d[nt][r][e];
-                    if (own_node) {
-                        // S5 on an owned node: eq. 12 spin blocks, in-term, R-term, divided by the plane's
-                        // z-weight because the Y task multiplies the whole XR entry by it
-                        const uint32_t lin = sb + (uint32_t)(q * n + xoc) * 128u + (fb0 & ~(uint32_t)(2 * ESZ - 1)) + 8 * r * ESZ;
-                        const T2 me = *reinterpret_cast<const T2*>(smem + swz(lin));
-                        const T2 ot = *reinterpret_cast<const T2*>(smem + swz(lin ^ 64u));
-                        const double own = ri ? (double)me.y : (double)me.x;
-                        const double osame = ri ? (double)ot.y : (double)ot.x, oflip = ri ? (double)ot.x : (double)ot.y;
-                        const double pot = fma(f0, own, fma(f2, osame, f3 * oflip));
-                        double s5 = fma(cin[r], own, sc.cHp * pot);
+                Val val;
+                val.a = sXWY * acc.d[nt][0][e];
+                val.b = NR == 2 ? sXWY * acc.d[nt][NR - 1][e] : (T)0;
+                if (own_node) {
+                    // S5 on an owned node: eq. 12 spin blocks, in-term, R-term, divided by the plane's
+                    // z-weight because the Y task multiplies the whole XR entry by it
+                    const double fd = Fs[xoc * 4 + spin], bx = Fs[xoc * 4 + 2], by = sgs * Fs[xoc * 4 + 3];
+                    const uint32_t lin = sb + (uint32_t)(q * n + xoc) * 128u + fb0;
+                    if constexpr (F64) {
+                        // own component ri of spin s; the other spin's same and other component
+                        const double own = ldu(lin), osame = ldu(lin ^ 64u), oflip = ldu(lin ^ 72u);
+                        // s = 0: (B_x - i B_y) u' ; s = 1: (B_x + i B_y) u' ; re: B_x c + sgs B_y d ; im: B_x d - sgs B_y c
+                        const double pot = fma(fd, own, fma(bx, osame, (ri ? -by : by) * oflip));
+                        double s5 = fma(cin, own, sc.cHp * pot);
+                        if (ar.useR) s5 = fma(cR, *reinterpret_cast<const double*>(smem + swz64(rb + (uint32_t)(q * P + xoc) * 128u + fb0)), s5);
+                        val.a = fma(s5, inv_wz, val.a);
+                    } else {
+                        const float2 me = ldu(lin), ot = ldu(lin ^ 64u);
+                        const double a = me.x, b = me.y, c = ot.x, d = ot.y;
+                        const double pre = fma(fd, a, fma(bx, c, by * d)), pim = fma(fd, b, fma(bx, d, -by * c));
+                        double sre = fma(cin, a, sc.cHp * pre), sim = fma(cin, b, sc.cHp * pim);
                         if (ar.useR) {
-                            const uint32_t rl = rb + (uint32_t)((q * P + xoc) * C + col0 + 8 * r) * 8u;
-                            s5 = fma(cR[r], *reinterpret_cast<const double*>(smem + swz(rl)), s5);
+                            // R is complex128: the (node, spin) row is 16 doubles = 128 bytes, vector vl at byte 16 vl
+                            const uint32_t rl = rb + (uint32_t)((q * P + xoc) * 2 + spin) * 128u + (uint32_t)vl * 16u;
+                            const double2 rv = *reinterpret_cast<const double2*>(smem + swz128(rl));
+                            sre = fma(cR, rv.x, sre); sim = fma(cR, rv.y, sim);
                         }
-                        val = fma((T)s5, inv_wz, val);
+                        val.a = fmaf((float)sre, inv_wz, val.a);
+                        val.b = fmaf((float)sim, inv_wz, val.b);
                     }
-                    if (live) XR[xoc * XP + 8 * r] = val;
+                }
+                if (live) {
+                    if constexpr (F64) XR[xoc * XPU] = val.a;
+                    else XR[xoc * XPU] = make_float2(val.a, val.b);
                 }
             }
         if (up) {
@@ -416,8 +456,8 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
     auto ytask = [&](int tp, uint32_t sb, T wz) {
         Acc<P, MODE> acc;
         acc.zero();
-        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, int r) { return lds(sb + ya[ks][h] + 8 * r * ESZ); });
-        const T* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / ESZ) + q * XP + col0;
+        contract<P, MODE>(acc, bf, t4, [&](int ks, int h) { return ldu(sb + ya[ks][h]); });
+        const U* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / 8) + q * XPU + upos;
         const bool zwrap = (g0 + tp) == ar.n1[2];
         const bool zp = HASPH && zwrap && ar.phd[2];
         const bool anyph = HASPH && ((q == P && xph) || yph || zp);    // warp-uniform
@@ -438,12 +478,12 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 const bool live = nt * 8 + 6 + e < n || yo < n;
                 const int yoc = live ? yo : 0;
                 const long long yq = nt == 0 ? (e == 0 ? yq0 : yq1) : (e == 0 ? yq8 : yq9);
-#pragma unroll
-                for (int r = 0; r < NR; ++r) {
-                    T val = wz * fma(sYWX, acc.d[nt][r][e], XR[(yoc * n) * XP + 8 * r]);
-                    if (anyph) val = conj_phase(val, yoc == P ? pr1 : pr0, yoc == P ? pi1 : pi0);
-                    if (live && vok[r]) red_add_t(pbase + yq + 8 * r, val);
-                }
+                const U xr = XR[(yoc * n) * XPU];
+                Val val;
+                if constexpr (F64) { val.a = wz * fma(sYWX, acc.d[nt][0][e], xr); val.b = 0; }
+                else { val.a = wz * fmaf(sYWX, acc.d[nt][0][e], xr.x); val.b = wz * fmaf(sYWX, acc.d[nt][NR - 1][e], xr.y); }
+                if (anyph) val = conj_phase(val, yoc == P ? pr1 : pr0, yoc == P ? pi1 : pi0);
+                if (live && vok) emit(pbase + yq, val);
             }
     };
 
@@ -470,7 +510,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
             Acc<P, MODE> acc;
             acc.zero();
             const uint32_t no = (uint32_t)i * 128u;
-            contract<P, MODE>(acc, bf, t4, [&](int ks, int h, int r) { return lds(zb[ks][h] + no + 8 * r * ESZ); });
+            contract<P, MODE>(acc, bf, t4, [&](int ks, int h) { return ldu(zb[ks][h] + no); });
             const T w = sc.W[0][i] * WYq;
             const bool anyph = HASPH && ((i == P && xph) || (q == P && yph) || zp);
             double pr0 = 1.0, pi0 = 0.0, pr1 = 1.0, pi1 = 0.0;          // conj phase of planes < P / of the wrapped top plane
@@ -490,12 +530,11 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                     const bool live = nt * 8 + 6 + e < n || ko < n;
                     const int koc = live ? ko : 0;
                     const long long zq = nt == 0 ? (e == 0 ? zq0 : zq1) : (e == 0 ? zq8 : zq9);
-#pragma unroll
-                    for (int r = 0; r < NR; ++r) {
-                        T val = w * acc.d[nt][r][e];
-                        if (anyph) val = conj_phase(val, koc == P ? pr1 : pr0, koc == P ? pi1 : pi0);
-                        if (live && vok[r]) red_add_t(nb + zq + 8 * r, val);
-                    }
+                    Val val;
+                    val.a = w * acc.d[nt][0][e];
+                    val.b = NR == 2 ? w * acc.d[nt][NR - 1][e] : (T)0;
+                    if (anyph) val = conj_phase(val, koc == P ? pr1 : pr0, koc == P ? pi1 : pi0);
+                    if (live && vok) emit(nb + zq, val);
                 }
         }
     };
@@ -601,15 +640,18 @@ static cudaError_t launch_mma_t(const chfsi_mesh* m, const CellArgs& a, cudaStre
     constexpr int BC = Cfg::C / 2;
     constexpr bool f32 = sizeof(T) == 4;
     const int nl[3] = {P + 1, P, 1};
+    const int sw64 = kSwizzle ? 64 : 0, sw128 = kSwizzle ? 128 : 0;
     // with a single cell in x the 2(P+1)-row box would not fit the x-line: such meshes always take the per-line path
     const int rows_full = ar.nc[0] > 1 ? 2 * (P + 1) : 2 * P;
     for (int i = 0; i < 3; ++i)
-        if (!make_map3(&mp.main[i], m, a.in, a.ld_in, a.nvec, BC, rows_full, nl[i], f32, kSwizzle)) return cudaErrorInvalidValue;
-    if (!make_map3(&mp.face[0], m, a.in, a.ld_in, a.nvec, BC, 2 * P, 1, f32, kSwizzle) ||
-        !make_map3(&mp.face[1], m, a.in, a.ld_in, a.nvec, BC, 2, 1, f32, kSwizzle) ||
-        !make_map3(&mp.face[2], m, a.in, a.ld_in, a.nvec, BC, 2, 1, f32, kSwizzle))
+        if (!make_map3(&mp.main[i], m, a.in, a.ld_in, a.nvec, BC, rows_full, nl[i], f32, sw64)) return cudaErrorInvalidValue;
+    if (!make_map3(&mp.face[0], m, a.in, a.ld_in, a.nvec, BC, 2 * P, 1, f32, sw64) ||
+        !make_map3(&mp.face[1], m, a.in, a.ld_in, a.nvec, BC, 2, 1, f32, sw64) ||
+        !make_map3(&mp.face[2], m, a.in, a.ld_in, a.nvec, BC, 2, 1, f32, sw64))
         return cudaErrorInvalidValue;
-    if (!make_map3(&mp.R, m, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, a.nvec, BC, 2 * P, P, ar.useR ? false : f32, kSwizzle) ||
+    // R is complex128 in every mode: its (node, spin) row is 128 bytes with complex64 iterates, 64 bytes with complex128 ones
+    if (!make_map3(&mp.R, m, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, a.nvec, BC, 2 * P, P, ar.useR ? false : f32,
+                   f32 ? sw128 : sw64) ||
         !make_mapF(&mp.F, m, P))
         return cudaErrorInvalidValue;
     if (a.flags & kMassIn) return cudaErrorInvalidValue;             // the residual S0 runs on the line-owned FP64 kernel

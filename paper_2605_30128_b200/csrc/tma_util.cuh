@@ -91,7 +91,7 @@ static inline EncodeFn get_encode() {
 // past the caller's allocation whatever ld and the chunk offset are), dim1 = the 2*N1x rows of one x-line, dim2 = the
 // N1y*N1z x-lines; box = box_cols reals x box_rows rows x box_lines lines.  f32: the multivector is complex64.
 static inline bool make_map3(CUtensorMap* map, const chfsi_mesh* m, const void* base, long long ld, int nvec, int box_cols,
-                             int box_rows, int box_lines, bool f32 = false, bool swizzle128 = false) {
+                             int box_rows, int box_lines, bool f32 = false, int swizzle_bytes = 0) {
     EncodeFn enc = get_encode();
     if (!enc) return false;
     const cuuint64_t n1x = (cuuint64_t)m->mc.n1[0];
@@ -101,7 +101,7 @@ static inline bool make_map3(CUtensorMap* map, const chfsi_mesh* m, const void* 
     cuuint32_t box[3] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows, (cuuint32_t)box_lines};
     cuuint32_t estr[3] = {1u, 1u, 1u};
     return enc(map, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), gdim,
-               gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+               gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
