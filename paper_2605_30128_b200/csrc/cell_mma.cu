@@ -66,7 +66,7 @@ struct MmaCfg {
     static constexpr int C = 2 * MROWS, NV = C / 4;          // real batch columns of the CTA: both spin components
     static constexpr int NR = MROWS / 8, KH = KSTEP / 4;     // fragment rows g + 8r, fragment k-halves
     static constexpr int KS = (n + KSTEP - 1) / KSTEP, NT = (n + 7) / 8;
-    static constexpr int NCW = 2 * n;                        // consumer warps: (index q in 0..p) x (spin)
+    static constexpr int NCW = n;                            // consumer warps: index q in 0..p; a warp runs both m-tiles
     static constexpr int THREADS = (NCW + 1) * 32;
     static constexpr int ESZ = (int)sizeof(T);
     static_assert(C * ESZ == 128, "one node of the CTA's columns is one 128-byte row");
@@ -167,46 +167,54 @@ struct Acc {
     }
 };
 
-// acc += K applied along the line whose 8-byte unit at element kmap(ks, h, t) is ld(ks, h): a double (FP64, fragment row g)
-// or a float2 = (fragment row g, fragment row g + 8) (TF32)
+// acc[mt] += K applied along the line whose 8-byte units at element kmap(ks, h, t) are ld(ks, h, u[2]) for the two m-tiles:
+// a double (FP64, fragment row g) or a float2 = (fragment row g, fragment row g + 8) (TF32)
 template <int P, int MODE, typename LD>
-__device__ __forceinline__ void contract(Acc<P, MODE>& acc, const BFrags<P, MODE>& bf, int t, LD ld) {
+__device__ __forceinline__ void contract(Acc<P, MODE> (&acc)[2], const BFrags<P, MODE>& bf, int t, LD ld) {
     using Cfg = MmaCfg<P, MODE>;
     using T = typename Cfg::T;
+    using U = typename std::conditional<MODE == MM_F64, double, float2>::type;
 #pragma unroll
     for (int ks = 0; ks < Cfg::KS; ++ks) {
-        T a[Cfg::NR][Cfg::KH];
+        T a[2][Cfg::NR][Cfg::KH];
 #pragma unroll
         for (int h = 0; h < Cfg::KH; ++h) {
             // the last k-step is only partly populated: lanes beyond the line contribute zeros
             const bool all = kmap<MODE>(ks, h, 3) < Cfg::n;
             const bool ok = all || kmap<MODE>(ks, h, t) < Cfg::n;
-            if constexpr (MODE == MM_F64) {
-                a[0][h] = ok ? ld(ks, h) : 0.0;
-            } else {
-                const float2 u = ok ? ld(ks, h) : make_float2(0.f, 0.f);
-                a[0][h] = u.x; a[1][h] = u.y;
+            U u[2];
+            if (ok) ld(ks, h, u);
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) {
+                if constexpr (MODE == MM_F64) {
+                    a[mt][0][h] = ok ? u[mt] : 0.0;
+                } else {
+                    a[mt][0][h] = ok ? u[mt].x : 0.f; a[mt][1][h] = ok ? u[mt].y : 0.f;
+                }
             }
         }
-        if constexpr (MODE == MM_F64) {
 #pragma unroll
-            for (int nt = 0; nt < Cfg::NT; ++nt) mma_f64(acc.d[nt], a[0][0], bf.hi[ks][nt][0]);
-        } else {
-            uint32_t ah[2][2], al[2][2];
+        for (int mt = 0; mt < 2; ++mt) {
+            if constexpr (MODE == MM_F64) {
 #pragma unroll
-            for (int r = 0; r < 2; ++r)
+                for (int nt = 0; nt < Cfg::NT; ++nt) mma_f64(acc[mt].d[nt], a[mt][0][0], bf.hi[ks][nt][0]);
+            } else {
+                uint32_t ah[2][2], al[2][2];
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    ah[r][h] = to_tf32(a[r][h]);
-                    if constexpr (MODE == MM_TF32X3) al[r][h] = to_tf32(a[r][h] - tf32_value(ah[r][h]));
+                for (int r = 0; r < 2; ++r)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        ah[r][h] = to_tf32(a[mt][r][h]);
+                        if constexpr (MODE == MM_TF32X3) al[r][h] = to_tf32(a[mt][r][h] - tf32_value(ah[r][h]));
+                    }
+#pragma unroll
+                for (int nt = 0; nt < Cfg::NT; ++nt) {
+                    if constexpr (MODE == MM_TF32X3) {
+                        mma_tf32(acc[mt].d[nt], al, bf.hi[ks][nt]);            // small terms first
+                        mma_tf32(acc[mt].d[nt], ah, bf.lo[ks][nt]);
+                    }
+                    mma_tf32(acc[mt].d[nt], ah, bf.hi[ks][nt]);
                 }
-#pragma unroll
-            for (int nt = 0; nt < Cfg::NT; ++nt) {
-                if constexpr (MODE == MM_TF32X3) {
-                    mma_tf32(acc.d[nt], al, bf.hi[ks][nt]);            // small terms first
-                    mma_tf32(acc.d[nt], ah, bf.lo[ks][nt]);
-                }
-                mma_tf32(acc.d[nt], ah, bf.hi[ks][nt]);
             }
         }
     }
@@ -295,27 +303,35 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
     }
 
     // ================================ consumers ================================
-    // warp = (index q in 0..p: row j of the X and Z tasks, x-position i of the Y task) x (m-tile mt: half of the CTA's vectors)
-    const int mt = warp & 1, q = warp >> 1;
+    // warp = index q in 0..p: row j of the X and Z tasks, x-position i of the Y task; it runs both m-tiles (mt = 0, 1: the two
+    // halves of the CTA's vectors), whose units sit 32 bytes apart in a node row
+    const int q = warp;
     const int g = lane >> 2, t4 = lane & 3;
     // the thread's 8-byte unit inside a node's 128-byte row: bit 3 = g & 1, spin (bit 6) = (g >> 1) & 1, chunk = 2 mt + (g >> 2)
     const int spin = (g >> 1) & 1;
-    const uint32_t fb0 = (uint32_t)(spin * 64 + (2 * mt + (g >> 2)) * 16 + (g & 1) * 8);
-    const int upos = (int)(fb0 >> 3);             // unit index inside the node (XR)
-    // TF32: unit = complex64 of vector vl; FP64: unit = the re (ri = 0) or im (ri = 1) part of vector vl
-    const int vl = F64 ? 2 * mt + (g >> 2) : 4 * mt + 2 * (g >> 2) + (g & 1);
+    const uint32_t fb0 = (uint32_t)(spin * 64 + (g >> 2) * 16 + (g & 1) * 8);       // m-tile 0; m-tile 1 is 32 bytes on
+    const int upos = (int)(fb0 >> 3);             // unit index inside the node (XR); m-tile 1: + 4
+    // TF32: unit = complex64 of vector vl; FP64: unit = the re (ri = 0) or im (ri = 1) part of vector vl; m-tile 1: vl + VSTEP
+    constexpr int VSTEP = F64 ? 2 : 4;
+    const int vl = F64 ? (g >> 2) : 2 * (g >> 2) + (g & 1);
     const int ri = F64 ? (g & 1) : 0;
     const double sgs = spin == 0 ? 1.0 : -1.0;    // sign of B_y in (B_x -+ i B_y)
     const int NTH = Cfg::NCW * 32;
     BFrags<P, MODE> bf;
     bf.init(sc, g, t4);
     const int v = chunk * Cfg::NV + vl;
-    const bool vok = FULLV || v < ar.nvec;
-    const double cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
-    const double cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
+    bool vok[2];
+    double cin[2], cR[2];
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt) {
+        vok[mt] = FULLV || v + VSTEP * mt < ar.nvec;
+        cin[mt] = (vok[mt] && ar.cin) ? __ldg(ar.cin + v + VSTEP * mt) : 0.0;
+        cR[mt] = (vok[mt] && ar.cR && ar.useR) ? __ldg(ar.cR + v + VSTEP * mt) : 0.0;
+    }
+    constexpr int OSTEP = 2 * VSTEP;              // scalars of T between the two m-tiles' outputs
     // `out` offsets in scalars of T: node I -> 4 ld I; spin -> 2 ld; vector v -> 2 v (+ ri)
     const long long XS = 4 * ar.ld_out, LS = (long long)ar.n1[0] * XS, PS = (long long)ar.n1[1] * LS;
-    const long long ocol0 = ((long long)spin * ar.ld_out + (vok ? v : 0)) * 2 + ri;
+    const long long ocol0 = ((long long)spin * ar.ld_out + (vok[0] ? v : 0)) * 2 + ri;
     T* const outp = reinterpret_cast<T*>(ar.out);
     auto xoff = [&](int i) { int gx = ex * P + i; if (gx == ar.n1[0]) gx = 0; return (long long)gx * XS; };
     auto yoff = [&](int j) { int gy = ey * P + j; if (gy == ar.n1[1]) gy = 0; return (long long)gy * LS; };
@@ -339,6 +355,12 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
             ya[ks][h] = (uint32_t)(kk * n + q) * 128u + fb0;
         }
     auto ldu = [&](uint32_t lin) { return *reinterpret_cast<const U*>(smem + swz64(lin)); };
+    // the units of both m-tiles at (m-tile 0) offset lin: bit 5 of lin is clear, so "+ 32" commutes with the swizzle as "^ 32"
+    auto ldu2 = [&](uint32_t lin, U (&u)[2]) {
+        const uint32_t a = swz64(lin);
+        u[0] = *reinterpret_cast<const U*>(smem + a);
+        u[1] = *reinterpret_cast<const U*>(smem + (a ^ 32u));
+    };
 
     // a complex output value held as d[0] = re, d[1] = im (TF32) or as the component ri of it (FP64, partner in lane ^ 4)
     struct Val { T a, b; };
@@ -362,7 +384,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
     auto xtask = [&](int tp, uint32_t sb, int rsl, int rpar, bool up, T inv_wz) {
         if (HASPH) {
             // Bloch phase on wrapped entries of the landed plane (x: node P of every line; y: line P; z: the whole wrapped
-            // plane), fixed up in place before any task reads the plane (boundary CTAs only); this warp fixes row q of its units
+            // plane), fixed up in place before any task reads the plane (boundary CTAs only); this warp fixes row q
             const bool wz = ar.phd[2] && (g0 + tp) == ar.n1[2];
             if (xph | yph | wz) {                                       // CTA-uniform
                 double br = 1.0, bi = 0.0;
@@ -375,15 +397,19 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                     double pr = br, pi = bi;
                     const bool fx = i == P && xph;
                     if (fx) { const double u = pr * ar.ph_re[0] - pi * ar.ph_im[0]; pi = pr * ar.ph_im[0] + pi * ar.ph_re[0]; pr = u; }
-                    U* e = reinterpret_cast<U*>(smem + swz64(sb + (uint32_t)(q * n + (valid ? i : 0)) * 128u + fb0));
-                    if constexpr (F64) {
-                        const double val = valid ? *e : 0.0;
-                        const double other = __shfl_xor_sync(0xffffffffu, val, 4);
-                        if (valid && (rowph || fx)) *e = fma(other, ri ? pi : -pi, val * pr);   // re' = re pr - im pi ; im' = im pr + re pi
-                    } else {
-                        if (valid && (rowph || fx)) {
-                            const float2 z = *e;
-                            *e = make_float2((float)fma((double)z.y, -pi, (double)z.x * pr), (float)fma((double)z.x, pi, (double)z.y * pr));
+                    const uint32_t ea = swz64(sb + (uint32_t)(q * n + (valid ? i : 0)) * 128u + fb0);
+#pragma unroll
+                    for (int mt = 0; mt < 2; ++mt) {
+                        U* e = reinterpret_cast<U*>(smem + (ea ^ (mt ? 32u : 0u)));
+                        if constexpr (F64) {
+                            const double val = valid ? *e : 0.0;
+                            const double other = __shfl_xor_sync(0xffffffffu, val, 4);
+                            if (valid && (rowph || fx)) *e = fma(other, ri ? pi : -pi, val * pr);   // re' = re pr - im pi ; im' = im pr + re pi
+                        } else {
+                            if (valid && (rowph || fx)) {
+                                const float2 z = *e;
+                                *e = make_float2((float)fma((double)z.y, -pi, (double)z.x * pr), (float)fma((double)z.x, pi, (double)z.y * pr));
+                            }
                         }
                     }
                 }
@@ -393,9 +419,9 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 __syncwarp();
             }
         }
-        Acc<P, MODE> acc;
-        acc.zero();
-        contract<P, MODE>(acc, bf, t4, [&](int ks, int h) { return ldu(sb + xa[ks][h]); });
+        Acc<P, MODE> acc[2];
+        acc[0].zero(); acc[1].zero();
+        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[2]) { ldu2(sb + xa[ks][h], u); });
         U* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / 8) + (q * n) * XPU + upos;
         const bool s5on = up && q < P;
         if (s5on) mbar_wait(&full_r[rsl], rpar);
@@ -410,40 +436,59 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 const bool live = nt * 8 + 6 + e < n || xo < n;          // compile-time true for fully populated n-tiles
                 const int xoc = live ? xo : 0;
                 const bool own_node = s5on && live && (nt * 8 + 6 + e < P || xoc < P);
-                Val val;
-                val.a = sXWY * acc.d[nt][0][e];
-                val.b = NR == 2 ? sXWY * acc.d[nt][NR - 1][e] : (T)0;
+                Val val[2];
+#pragma unroll
+                for (int mt = 0; mt < 2; ++mt) {
+                    val[mt].a = sXWY * acc[mt].d[nt][0][e];
+                    val[mt].b = NR == 2 ? sXWY * acc[mt].d[nt][NR - 1][e] : (T)0;
+                }
                 if (own_node) {
                     // S5 on an owned node: eq. 12 spin blocks, in-term, R-term, divided by the plane's
                     // z-weight because the Y task multiplies the whole XR entry by it
                     const double fd = Fs[xoc * 4 + spin], bx = Fs[xoc * 4 + 2], by = sgs * Fs[xoc * 4 + 3];
                     const uint32_t lin = sb + (uint32_t)(q * n + xoc) * 128u + fb0;
+                    U me[2], ot[2];
+                    ldu2(lin, me);
+                    ldu2(lin ^ 64u, ot);
                     if constexpr (F64) {
-                        // own component ri of spin s; the other spin's same and other component
-                        const double own = ldu(lin), osame = ldu(lin ^ 64u), oflip = ldu(lin ^ 72u);
-                        // s = 0: (B_x - i B_y) u' ; s = 1: (B_x + i B_y) u' ; re: B_x c + sgs B_y d ; im: B_x d - sgs B_y c
-                        const double pot = fma(fd, own, fma(bx, osame, (ri ? -by : by) * oflip));
-                        double s5 = fma(cin, own, sc.cHp * pot);
-                        if (ar.useR) s5 = fma(cR, *reinterpret_cast<const double*>(smem + swz64(rb + (uint32_t)(q * P + xoc) * 128u + fb0)), s5);
-                        val.a = fma(s5, inv_wz, val.a);
-                    } else {
-                        const float2 me = ldu(lin), ot = ldu(lin ^ 64u);
-                        const double a = me.x, b = me.y, c = ot.x, d = ot.y;
-                        const double pre = fma(fd, a, fma(bx, c, by * d)), pim = fma(fd, b, fma(bx, d, -by * c));
-                        double sre = fma(cin, a, sc.cHp * pre), sim = fma(cin, b, sc.cHp * pim);
-                        if (ar.useR) {
-                            // R is complex128: the (node, spin) row is 16 doubles = 128 bytes, vector vl at byte 16 vl
-                            const uint32_t rl = rb + (uint32_t)((q * P + xoc) * 2 + spin) * 128u + (uint32_t)vl * 16u;
-                            const double2 rv = *reinterpret_cast<const double2*>(smem + swz128(rl));
-                            sre = fma(cR, rv.x, sre); sim = fma(cR, rv.y, sim);
+                        // own component ri of spin s; the other spin's same (ot) and other (of) component
+                        U of[2];
+                        ldu2(lin ^ 72u, of);
+                        const uint32_t rs0 = swz64(rb + (uint32_t)(q * P + xoc) * 128u + fb0);
+#pragma unroll
+                        for (int mt = 0; mt < 2; ++mt) {
+                            // s = 0: (B_x - i B_y) u' ; s = 1: (B_x + i B_y) u' ; re: B_x c + sgs B_y d ; im: B_x d - sgs B_y c
+                            const double pot = fma(fd, me[mt], fma(bx, ot[mt], (ri ? -by : by) * of[mt]));
+                            double s5 = fma(cin[mt], me[mt], sc.cHp * pot);
+                            if (ar.useR) s5 = fma(cR[mt], *reinterpret_cast<const double*>(smem + (rs0 ^ (mt ? 32u : 0u))), s5);
+                            val[mt].a = fma(s5, inv_wz, val[mt].a);
                         }
-                        val.a = fmaf((float)sre, inv_wz, val.a);
-                        val.b = fmaf((float)sim, inv_wz, val.b);
+                    } else {
+                        // R is complex128: the (node, spin) row is 16 doubles = 128 bytes, vector vl at byte 16 vl; m-tile 1 is
+                        // 4 vectors = 64 bytes on (bit 6 of the offset is clear for m-tile 0)
+                        const uint32_t rs0 = swz128(rb + (uint32_t)((q * P + xoc) * 2 + spin) * 128u + (uint32_t)vl * 16u);
+                        // FP32 arithmetic ("pointwise terms stay FP32", A7); the R-term is formed in FP64 and rounded once
+                        const float fdf = (float)fd, bxf = (float)bx, byf = (float)by, chp = (float)sc.cHp;
+#pragma unroll
+                        for (int mt = 0; mt < 2; ++mt) {
+                            const float a = me[mt].x, b = me[mt].y, c = ot[mt].x, d = ot[mt].y;
+                            const float pre = fmaf(fdf, a, fmaf(bxf, c, byf * d)), pim = fmaf(fdf, b, fmaf(bxf, d, -byf * c));
+                            float sre = fmaf((float)cin[mt], a, chp * pre), sim = fmaf((float)cin[mt], b, chp * pim);
+                            if (ar.useR) {
+                                const double2 rv = *reinterpret_cast<const double2*>(smem + (rs0 ^ (mt ? 64u : 0u)));
+                                sre += (float)(cR[mt] * rv.x); sim += (float)(cR[mt] * rv.y);
+                            }
+                            val[mt].a = fmaf(sre, inv_wz, val[mt].a);
+                            val[mt].b = fmaf(sim, inv_wz, val[mt].b);
+                        }
                     }
                 }
                 if (live) {
-                    if constexpr (F64) XR[xoc * XPU] = val.a;
-                    else XR[xoc * XPU] = make_float2(val.a, val.b);
+#pragma unroll
+                    for (int mt = 0; mt < 2; ++mt) {
+                        if constexpr (F64) XR[xoc * XPU + 4 * mt] = val[mt].a;
+                        else XR[xoc * XPU + 4 * mt] = make_float2(val[mt].a, val[mt].b);
+                    }
                 }
             }
         if (up) {
@@ -454,9 +499,9 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
 
     // ---- Y task of plane tp: y-contraction at x-position q, + XR (x part and S5), times the plane's z-weight -> RED to out
     auto ytask = [&](int tp, uint32_t sb, T wz) {
-        Acc<P, MODE> acc;
-        acc.zero();
-        contract<P, MODE>(acc, bf, t4, [&](int ks, int h) { return ldu(sb + ya[ks][h]); });
+        Acc<P, MODE> acc[2];
+        acc[0].zero(); acc[1].zero();
+        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[2]) { ldu2(sb + ya[ks][h], u); });
         const U* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / 8) + q * XPU + upos;
         const bool zwrap = (g0 + tp) == ar.n1[2];
         const bool zp = HASPH && zwrap && ar.phd[2];
@@ -469,22 +514,31 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
             if (yph) { pr1 = pr0 * ar.ph_re[1] - pi0 * ar.ph_im[1]; pi1 = pr0 * ar.ph_im[1] + pi0 * ar.ph_re[1]; }
         }
         T* const pbase = outp + zoff(g0 + tp) + xq_self;
+        auto outputs = [&](auto ph) {
+            constexpr bool PH = decltype(ph)::value;
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt)
+            for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                if (nt * 8 + e >= n) continue;
-                const int yo = nt * 8 + 2 * t4 + e;
-                const bool live = nt * 8 + 6 + e < n || yo < n;
-                const int yoc = live ? yo : 0;
-                const long long yq = nt == 0 ? (e == 0 ? yq0 : yq1) : (e == 0 ? yq8 : yq9);
-                const U xr = XR[(yoc * n) * XPU];
-                Val val;
-                if constexpr (F64) { val.a = wz * fma(sYWX, acc.d[nt][0][e], xr); val.b = 0; }
-                else { val.a = wz * fmaf(sYWX, acc.d[nt][0][e], xr.x); val.b = wz * fmaf(sYWX, acc.d[nt][NR - 1][e], xr.y); }
-                if (anyph) val = conj_phase(val, yoc == P ? pr1 : pr0, yoc == P ? pi1 : pi0);
-                if (live && vok) emit(pbase + yq, val);
-            }
+                for (int e = 0; e < 2; ++e) {
+                    if (nt * 8 + e >= n) continue;
+                    const int yo = nt * 8 + 2 * t4 + e;
+                    const bool live = nt * 8 + 6 + e < n || yo < n;
+                    const int yoc = live ? yo : 0;
+                    const long long yq = nt == 0 ? (e == 0 ? yq0 : yq1) : (e == 0 ? yq8 : yq9);
+#pragma unroll
+                    for (int mt = 0; mt < 2; ++mt) {
+                        const U xr = XR[(yoc * n) * XPU + 4 * mt];
+                        Val val;
+                        if constexpr (F64) { val.a = wz * fma(sYWX, acc[mt].d[nt][0][e], xr); val.b = 0; }
+                        else { val.a = wz * fmaf(sYWX, acc[mt].d[nt][0][e], xr.x); val.b = wz * fmaf(sYWX, acc[mt].d[nt][NR - 1][e], xr.y); }
+                        if constexpr (PH) val = conj_phase(val, yoc == P ? pr1 : pr0, yoc == P ? pi1 : pi0);
+                        if (live && vok[mt]) emit(pbase + yq + OSTEP * mt, val);
+                    }
+                }
+        };
+        // a real (warp-uniform) branch: the phase arithmetic must not be if-converted into the common path
+        if (anyph) outputs(std::true_type{});
+        else outputs(std::false_type{});
     };
 
     // ---- Z task of the cell whose planes sit in ring slots sl0, sl0+1, ... (mod S), first plane tb: z-contraction for the
@@ -507,10 +561,10 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
         const long long zq9 = zoff(g0 + tb + (9 + 2 * t4 < n ? 9 + 2 * t4 : 0)) + zrow;
 #pragma unroll 1
         for (int i = 0; i < n; ++i) {
-            Acc<P, MODE> acc;
-            acc.zero();
+            Acc<P, MODE> acc[2];
+            acc[0].zero(); acc[1].zero();
             const uint32_t no = (uint32_t)i * 128u;
-            contract<P, MODE>(acc, bf, t4, [&](int ks, int h) { return ldu(zb[ks][h] + no); });
+            contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[2]) { ldu2(zb[ks][h] + no, u); });
             const T w = sc.W[0][i] * WYq;
             const bool anyph = HASPH && ((i == P && xph) || (q == P && yph) || zp);
             double pr0 = 1.0, pi0 = 0.0, pr1 = 1.0, pi1 = 0.0;          // conj phase of planes < P / of the wrapped top plane
@@ -521,21 +575,29 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 if (zp) { pr1 = pr0 * ar.ph_re[2] - pi0 * ar.ph_im[2]; pi1 = pr0 * ar.ph_im[2] + pi0 * ar.ph_re[2]; }
             }
             T* const nb = outp + xoff(i);
+            auto outputs = [&](auto ph) {
+                constexpr bool PH = decltype(ph)::value;
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt)
+                for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    if (nt * 8 + e >= n) continue;
-                    const int ko = nt * 8 + 2 * t4 + e;
-                    const bool live = nt * 8 + 6 + e < n || ko < n;
-                    const int koc = live ? ko : 0;
-                    const long long zq = nt == 0 ? (e == 0 ? zq0 : zq1) : (e == 0 ? zq8 : zq9);
-                    Val val;
-                    val.a = w * acc.d[nt][0][e];
-                    val.b = NR == 2 ? w * acc.d[nt][NR - 1][e] : (T)0;
-                    if (anyph) val = conj_phase(val, koc == P ? pr1 : pr0, koc == P ? pi1 : pi0);
-                    if (live && vok) emit(nb + zq, val);
-                }
+                    for (int e = 0; e < 2; ++e) {
+                        if (nt * 8 + e >= n) continue;
+                        const int ko = nt * 8 + 2 * t4 + e;
+                        const bool live = nt * 8 + 6 + e < n || ko < n;
+                        const int koc = live ? ko : 0;
+                        const long long zq = nt == 0 ? (e == 0 ? zq0 : zq1) : (e == 0 ? zq8 : zq9);
+#pragma unroll
+                        for (int mt = 0; mt < 2; ++mt) {
+                            Val val;
+                            val.a = w * acc[mt].d[nt][0][e];
+                            val.b = NR == 2 ? w * acc[mt].d[nt][NR - 1][e] : (T)0;
+                            if constexpr (PH) val = conj_phase(val, koc == P ? pr1 : pr0, koc == P ? pi1 : pi0);
+                            if (live && vok[mt]) emit(nb + zq + OSTEP * mt, val);
+                        }
+                    }
+            };
+            if (anyph) outputs(std::true_type{});
+            else outputs(std::false_type{});
         }
     };
 
