@@ -306,7 +306,7 @@ def test_config1_full_size_sampled_columns(env):
 # ------------------------------------------------------------------------------- error behaviour (include/chfsi.h)
 def test_error_codes_on_device_calls(env):
     """Every call returns a status and leaves the outputs alone on error: ESTATE before ham_set, EINVAL for bad
-    degree / bounds / leading dimension / chunk / workspace / missing Lambda, EUNSUPPORTED for the TF32 modes."""
+    degree / bounds / leading dimension / chunk / workspace / missing Lambda, EUNSUPPORTED for the complex64-iterate modes outside eq. 11."""
     torch, fo, B = env
     cfg = inp.tiny_config(ncell=2, p=4, L=4.0, nvec=8, natoms=1, nproj=4)
     mesh = B.chfsi_mesh_create(cfg.ncell, cfg.L, cfg.p, cfg.kfrac, 0)
@@ -341,7 +341,11 @@ def test_error_codes_on_device_calls(env):
         assert filt(lam=None) == B.EINVAL                            # eq. 11 needs Lambda
         assert filt(work=work[:1024]) == B.EINVAL                    # workspace too small
         assert filt(work=work[8:]) == B.EINVAL                       # workspace not 256-byte aligned
-        assert filt(prec=B.TF32) == B.EUNSUPPORTED and filt(prec=B.TF32X3) == B.EUNSUPPORTED
+        # the complex64-iterate modes exist only inside eq. 11: EUNSUPPORTED with eq. 10 and in chfsi_apply_H
+        for pr in (B.TF32, B.TF32X3, B.FP32_STORED):
+            assert filt(prec=pr, recur=B.RECUR_STANDARD, lam=None) == B.EUNSUPPORTED
+            assert status(B.chfsi_apply_H, mesh, pr, X, Y, work) == B.EUNSUPPORTED
+        assert filt(prec=7) == B.EINVAL                              # unknown precision
         assert status(B.chfsi_apply_H, mesh, B.FP64, X, X, work) == B.EINVAL      # apply_H cannot alias
         torch.cuda.synchronize()
         assert bool((Y == 3.0).all())                                # failed calls wrote nothing
