@@ -197,6 +197,24 @@ chfsi_status chfsi_bfp_gather_encode(int nbits, const void* X, int complex_bytes
 chfsi_status chfsi_bfp_decode_scatter_add(int nbits, const void* src_stream, const long long* rows, long long nrows,
                                           int nvec, void* Y, int complex_bytes, long long ld, void* cuda_stream);
 
+/* ---- Rayleigh-Ritz pieces around the filter (Algorithm 1 lines 6-8) -------------
+ * chfsi_rr_project (RR-Proj): S = A^H diag(w) B, S: device, nvec x nvec complex128, row-major, overwritten.  A, B: device,
+ *   complex128, nrows rows, leading dimensions lda, ldb.  use_mass != 0: w = the node masses (row 2 I + alpha carries m_I,
+ *   nrows must be 2 * nnodes): with A = B = Y it is Y^H M Y, with B = M^-1 H Y (chfsi_apply_H) it is Y^H H Y; use_mass = 0:
+ *   w = 1 and mesh may be NULL.  hermitian != 0: only the tiles on and above the diagonal are computed and the rest is
+ *   mirrored (the caller asserts that the exact S is Hermitian); the diagonal is returned exactly real.  FP64.
+ * chfsi_rr_rotate (RR-SR): Yout = Y Q.  prec CHFSI_FP32: the paper's mixed precision, "Y Q_non-diag is evaluated in FP32
+ *   arithmetic, while Y Q_diag is computed in FP64" (Y and the off-diagonal of Q are rounded to complex64, products and
+ *   accumulation in FP32, the result widened and added to Y Q_diag).  prec CHFSI_FP64: all FP64.  Q: device, nvec x nvec
+ *   complex128, row-major.  Y and Yout must be distinct.  work: device scratch of chfsi_rr_rotate_workspace_bytes(nvec),
+ *   256-byte aligned.  Diagonalising the projected pencil (RR-diag, ELPA in the paper) is left to the caller.
+ * EINVAL: bad sizes / leading dimensions / alignment / NULL; EUNSUPPORTED: other precisions. */
+chfsi_status chfsi_rr_project(const chfsi_mesh* mesh, long long nrows, int nvec, const void* A, long long lda,
+                              const void* B, long long ldb, int use_mass, int hermitian, void* S, void* cuda_stream);
+chfsi_status chfsi_rr_rotate_workspace_bytes(int nvec, size_t* bytes);
+chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q,
+                             void* Yout, long long ldo, void* work, size_t work_bytes, void* cuda_stream);
+
 const char* chfsi_last_error(void);     /* thread-local; never NULL */
 const char* chfsi_version(void);
 

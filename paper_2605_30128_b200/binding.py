@@ -26,6 +26,7 @@ EXPORTS = [
     "chfsi_profile_enable", "chfsi_profile_read",
     "chfsi_bfp_stream_bytes", "chfsi_bfp_encode", "chfsi_bfp_decode", "chfsi_bfp_gather_encode",
     "chfsi_bfp_decode_scatter_add",
+    "chfsi_rr_project", "chfsi_rr_rotate_workspace_bytes", "chfsi_rr_rotate",
     "chfsi_last_launch_count", "chfsi_last_error", "chfsi_version",
 ]
 
@@ -67,6 +68,9 @@ def lib() -> C.CDLL:
     L.chfsi_bfp_decode.argtypes = [C.c_int, vp, C.c_longlong, vp, vp]
     L.chfsi_bfp_gather_encode.argtypes = [C.c_int, vp, C.c_int, C.c_longlong, C.c_int, vp, C.c_longlong, vp, vp]
     L.chfsi_bfp_decode_scatter_add.argtypes = [C.c_int, vp, vp, C.c_longlong, C.c_int, vp, C.c_int, C.c_longlong, vp]
+    L.chfsi_rr_project.argtypes = [vp, C.c_longlong, C.c_int, vp, C.c_longlong, vp, C.c_longlong, C.c_int, C.c_int, vp, vp]
+    L.chfsi_rr_rotate_workspace_bytes.argtypes = [C.c_int, C.POINTER(C.c_size_t)]
+    L.chfsi_rr_rotate.argtypes = [C.c_int, C.c_longlong, C.c_int, vp, C.c_longlong, vp, vp, C.c_longlong, vp, C.c_size_t, vp]
     for name in EXPORTS:
         if name not in ("chfsi_last_launch_count", "chfsi_last_error", "chfsi_version"):
             getattr(L, name).restype = C.c_int
@@ -232,3 +236,25 @@ def chfsi_bfp_gather_encode(nbits, X, rows, dst, stream=None):
 def chfsi_bfp_decode_scatter_add(nbits, src, rows, Y, stream=None):
     _check(lib().chfsi_bfp_decode_scatter_add(int(nbits), _ptr(src), _ptr(rows), rows.numel(), Y.shape[1], _ptr(Y),
                                               Y.element_size(), Y.stride(0), _stream(stream)))
+
+
+# ---- Rayleigh-Ritz pieces --------------------------------------------------------
+def chfsi_rr_project(mesh, A, B, S, use_mass=True, hermitian=True, stream=None):
+    """A, B: torch complex128 CUDA tensors [..., ld] viewed as [nrows, ld]; S: torch complex128 [nvec, nvec]."""
+    nvec = S.shape[0]
+    nrows = A.numel() // A.shape[-1]
+    _check(lib().chfsi_rr_project(mesh, nrows, nvec, _ptr(A), A.stride(-2), _ptr(B), B.stride(-2), int(bool(use_mass)),
+                                  int(bool(hermitian)), _ptr(S), _stream(stream)))
+
+
+def chfsi_rr_rotate_workspace_bytes(nvec) -> int:
+    b = C.c_size_t()
+    _check(lib().chfsi_rr_rotate_workspace_bytes(int(nvec), C.byref(b)))
+    return b.value
+
+
+def chfsi_rr_rotate(prec, Y, Q, Yout, work, stream=None):
+    nvec = Q.shape[0]
+    nrows = Y.numel() // Y.shape[-1]
+    _check(lib().chfsi_rr_rotate(int(prec), nrows, nvec, _ptr(Y), Y.stride(-2), _ptr(Q), _ptr(Yout), Yout.stride(-2), _ptr(work),
+                                 work.numel(), _stream(stream)))
