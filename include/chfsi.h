@@ -215,6 +215,12 @@ chfsi_status chfsi_rr_rotate_workspace_bytes(int nvec, size_t* bytes);
 chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q,
                              void* Yout, long long ldo, void* work, size_t work_bytes, void* cuda_stream);
 
+/* ---- measurement aid: issue-rate peaks of the FMA and mma.sync pipes ------------------------------
+ * Runs four register-resident micro-kernels on `device` (one 512-thread CTA per SM, a few milliseconds each, synchronises)
+ * and returns TFLOP/s (2 flop per FMA) in tflops[0..3]: FP64 FMA, FP32 FMA, mma.m8n8k4.f64, mma.m16n8k8.tf32.  bench.py
+ * reports them as the "alu" / tensor roofs of the kernels that are not HBM-bound.  EINVAL: NULL; ECUDA / ENOMEM. */
+chfsi_status chfsi_measure_pipe_peaks(int device, double* tflops);
+
 const char* chfsi_last_error(void);     /* thread-local; never NULL */
 const char* chfsi_version(void);
 

@@ -26,7 +26,7 @@ EXPORTS = [
     "chfsi_profile_enable", "chfsi_profile_read",
     "chfsi_bfp_stream_bytes", "chfsi_bfp_encode", "chfsi_bfp_decode", "chfsi_bfp_gather_encode",
     "chfsi_bfp_decode_scatter_add",
-    "chfsi_rr_project", "chfsi_rr_rotate_workspace_bytes", "chfsi_rr_rotate",
+    "chfsi_rr_project", "chfsi_rr_rotate_workspace_bytes", "chfsi_rr_rotate", "chfsi_measure_pipe_peaks",
     "chfsi_last_launch_count", "chfsi_last_error", "chfsi_version",
 ]
 
@@ -71,6 +71,7 @@ def lib() -> C.CDLL:
     L.chfsi_rr_project.argtypes = [vp, C.c_longlong, C.c_int, vp, C.c_longlong, vp, C.c_longlong, C.c_int, C.c_int, vp, vp]
     L.chfsi_rr_rotate_workspace_bytes.argtypes = [C.c_int, C.POINTER(C.c_size_t)]
     L.chfsi_rr_rotate.argtypes = [C.c_int, C.c_longlong, C.c_int, vp, C.c_longlong, vp, vp, C.c_longlong, vp, C.c_size_t, vp]
+    L.chfsi_measure_pipe_peaks.argtypes = [C.c_int, dp]
     for name in EXPORTS:
         if name not in ("chfsi_last_launch_count", "chfsi_last_error", "chfsi_version"):
             getattr(L, name).restype = C.c_int
@@ -258,3 +259,10 @@ def chfsi_rr_rotate(prec, Y, Q, Yout, work, stream=None):
     nrows = Y.numel() // Y.shape[-1]
     _check(lib().chfsi_rr_rotate(int(prec), nrows, nvec, _ptr(Y), Y.stride(-2), _ptr(Q), _ptr(Yout), Yout.stride(-2), _ptr(work),
                                  work.numel(), _stream(stream)))
+
+
+def chfsi_measure_pipe_peaks(device=0) -> dict:
+    """TFLOP/s of the FP64 FMA, FP32 FMA, mma.m8n8k4.f64 and mma.m16n8k8.tf32 pipes, measured now on `device`."""
+    out = (C.c_double * 4)()
+    _check(lib().chfsi_measure_pipe_peaks(int(device), out))
+    return {"fp64_fma": out[0], "fp32_fma": out[1], "fp64_mma": out[2], "tf32_mma": out[3]}

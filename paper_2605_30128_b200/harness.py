@@ -101,14 +101,25 @@ class GpuProblem:
         th = np.linalg.eigvalsh(T)
         return float(th[0]), float(th[-1] + beta)
 
-    def rayleigh_ritz(self, Y):
-        """Alg. 1 lines 6-9: Y^H H Y Q = Y^H M Y Q Lambda; returns (Y Q, Lambda)."""
+    def rayleigh_ritz(self, Y, lib_rr=None):
+        """Alg. 1 lines 6-9: Y^H H Y Q = Y^H M Y Q Lambda; returns (Y Q, Lambda).  lib_rr = None: projection and rotation
+        with torch dense algebra; lib_rr = B.FP64 / B.FP32: with the library's chfsi_rr_project and chfsi_rr_rotate (FP32 =
+        the paper's FP64-diagonal + FP32-off-diagonal rotation).  The small dense eigenproblem stays in torch."""
         t = self.torch
         M2 = 2 * self.nnodes
         nv = Y.shape[-1]
-        HY = self.mass[:, None, None] * self.apply_MinvH(Y)
-        Hs = Y.reshape(M2, nv).conj().T @ HY.reshape(M2, nv)
-        Ss = self.m_inner(Y, Y)
+        if lib_rr is not None:
+            Yc = Y.contiguous()
+            HYm = self.apply_MinvH(Yc)
+            Hs = t.empty((nv, nv), dtype=t.complex128, device=Y.device)
+            Ss = t.empty_like(Hs)
+            B.chfsi_rr_project(self.mesh, Yc, HYm, Hs)
+            B.chfsi_rr_project(self.mesh, Yc, Yc, Ss)
+            del HYm
+        else:
+            HY = self.mass[:, None, None] * self.apply_MinvH(Y)
+            Hs = Y.reshape(M2, nv).conj().T @ HY.reshape(M2, nv)
+            Ss = self.m_inner(Y, Y)
         Hs = 0.5 * (Hs + Hs.conj().T)
         Ss = 0.5 * (Ss + Ss.conj().T)
         Lc = t.linalg.cholesky(Ss)
@@ -116,6 +127,11 @@ class GpuProblem:
         A = t.linalg.solve_triangular(Lc, A.conj().T, upper=False).conj().T
         lam, U = t.linalg.eigh(0.5 * (A + A.conj().T))
         Q = t.linalg.solve_triangular(Lc.conj().T, U, upper=True)
+        if lib_rr is not None:
+            Xn = t.empty_like(Yc)
+            wk = t.empty(B.chfsi_rr_rotate_workspace_bytes(nv), dtype=t.uint8, device=Y.device)
+            B.chfsi_rr_rotate(lib_rr, Yc, Q.contiguous(), Xn, wk)
+            return Xn, lam.cpu().numpy()
         Xn = (Y.reshape(M2, nv) @ Q).reshape(self.nnodes, 2, nv).contiguous()
         return Xn, lam.cpu().numpy()
 
@@ -126,9 +142,9 @@ class GpuProblem:
         return t.sqrt((R.abs() ** 2).sum(dim=(0, 1))).cpu().numpy()
 
     def subspace_iteration(self, X0, degree, b, passes, tol=1e-6, n_check=None, prec=B.FP64,
-                           recur=B.RECUR_RESIDUAL, chunk=0):
-        """Algorithm 1 with the GPU filter in `prec`; RR and residuals in FP64.  Returns (X, lam, hist)."""
-        X, lam = self.rayleigh_ritz(X0)
+                           recur=B.RECUR_RESIDUAL, chunk=0, lib_rr=None):
+        """Algorithm 1 with the GPU filter in `prec`; RR and residuals in FP64 (lib_rr: see rayleigh_ritz).  Returns (X, lam, hist)."""
+        X, lam = self.rayleigh_ritz(X0, lib_rr)
         nv = X.shape[-1]
         n_check = n_check or (3 * nv) // 4
         hist = []
@@ -139,5 +155,5 @@ class GpuProblem:
             if hist[-1] <= tol:
                 break
             Y = self.cheb_filter(X, lam, degree, float(lam[-1]), b, float(lam[0]), prec, recur, chunk)
-            X, lam = self.rayleigh_ritz(Y)
+            X, lam = self.rayleigh_ritz(Y, lib_rr)
         return X, lam, hist

@@ -135,8 +135,8 @@ def test_config3_full_size_p8_bloch_chunked(env):
 
 
 # ------------------------------------------------------------------------------- eigenvalue criterion
-def _converge(pb, X0, degree, b, prec, tol, n_check, max_passes):
-    X, lam, hist = pb.subspace_iteration(X0, degree, b, max_passes, tol=tol, n_check=n_check, prec=prec)
+def _converge(pb, X0, degree, b, prec, tol, n_check, max_passes, lib_rr=None):
+    X, lam, hist = pb.subspace_iteration(X0, degree, b, max_passes, tol=tol, n_check=n_check, prec=prec, lib_rr=lib_rr)
     return lam, hist
 
 
@@ -158,11 +158,15 @@ def test_eigenvalues_fp32_filter_vs_dense_oracle(env):
         _, b = pb.lanczos_bounds(10)
         X0 = torch.from_numpy(inp.make_vectors(cfg.nnodes, cfg.nvec, seed=0)).cuda()
         n_check = 18
-        for prec in (B.FP32, B.FP64):
-            lam, hist = _converge(pb, X0, cfg.degree, b, prec, 1e-6, n_check, 200)
-            assert hist[-1] <= 1e-6, (prec, hist[-5:])
+        # every inexact mode, incl. single-pass TF32 (its per-call error is 1e-3: what it is held to is this), and
+        # the library's own Rayleigh-Ritz kernels with the paper's mixed-precision rotation
+        for prec, lib_rr in ((B.FP32, None), (B.FP64, None), (B.FP32_STORED, None), (B.TF32X3, None), (B.TF32, None),
+                             (B.FP64, B.FP64), (B.TF32, B.FP32)):
+            lam, hist = _converge(pb, X0, cfg.degree, b, prec, 1e-6, n_check, 200, lib_rr=lib_rr)
+            assert hist[-1] <= 1e-6, (prec, lib_rr, hist[-5:])
             err = np.max(np.abs(lam[:n_check] - exact[:n_check]))
-            assert err < 1e-8, (prec, err)
+            print(f"prec {prec} lib_rr {lib_rr}: {len(hist)} passes, max eigenvalue error {err:.2e} Ha")
+            assert err < 1e-8, (prec, lib_rr, err)
     finally:
         pb.close()
 
@@ -197,8 +201,11 @@ def test_eigenvalues_config2_mesh_fp32_vs_exact_free_electron_spectrum(env):
 
 
 def test_eigenvalues_config2_fp32_vs_fp64_filter(env):
-    """configs[2]'s Hamiltonian at full size, 64-vector block: the eigenvalues reached with the FP32-inexact filter
-    agree within 1e-8 Ha with those reached with the FP64 filter (itself held to 1e-11 per call above)."""
+    """configs[2]'s Hamiltonian at full size, 64-vector block: the eigenvalues reached with the inexact filters (FP32
+    product, FP32-stored, single-pass TF32) agree within 1e-8 Ha with those reached with the FP64 filter (itself held to
+    1e-11 per call above).  An oracle-side subspace iteration at this size (~3.5 s per column and filter call on the
+    host) is out of reach of a test; the oracle-referenced eigenvalue checks are the dense pencil above and the exact
+    free-electron spectrum on this mesh."""
     torch, fo, B = env
     from paper_2605_30128_b200.harness import GpuProblem
     cfg = inp.CONFIGS[2]
@@ -207,9 +214,13 @@ def test_eigenvalues_config2_fp32_vs_fp64_filter(env):
         _, b = pb.lanczos_bounds(10)
         nvec, n_check = 64, 32
         X0 = torch.from_numpy(inp.make_vectors(cfg.nnodes, nvec, seed=0)).cuda()
-        l32, h32 = _converge(pb, X0, cfg.degree, b, B.FP32, 3e-6, n_check, 150)
         l64, h64 = _converge(pb, X0, cfg.degree, b, B.FP64, 3e-6, n_check, 150)
-        assert h32[-1] <= 3e-6 and h64[-1] <= 3e-6, (h32[-3:], h64[-3:])
-        assert np.max(np.abs(l32[:n_check] - l64[:n_check])) < 1e-8
+        assert h64[-1] <= 3e-6, h64[-3:]
+        for prec in (B.FP32, B.FP32_STORED, B.TF32):
+            lx, hx = _converge(pb, X0, cfg.degree, b, prec, 3e-6, n_check, 150)
+            assert hx[-1] <= 3e-6, (prec, hx[-3:])
+            err = np.max(np.abs(lx[:n_check] - l64[:n_check]))
+            print(f"c2 prec {prec}: {len(hx)} passes (FP64: {len(h64)}), max eigenvalue difference {err:.2e} Ha")
+            assert err < 1e-8, (prec, err)
     finally:
         pb.close()
