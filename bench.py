@@ -318,6 +318,72 @@ def all_configs_table(torch, B, device, peak):
     return rows
 
 
+
+def extra_kernels(torch, B, device, hbm_peak, pipe):
+    """Rows for the NEXT components that are not part of a filter step: the BFP codec (HBM-bound) and the Rayleigh-Ritz
+    projection / rotation (FMA-pipe bound; the roof is the issue rate measured in this run by chfsi_measure_pipe_peaks)."""
+    dev = f"cuda:{device}"
+    rows = []
+
+    def timed(fn, reps=3):
+        fn(); torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record(); torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    # ---- BFP codec on a face-slab stream of 2^28 FP32 values (1 GiB in): algorithmic bytes = 16 B in + n_bits/2 B out per block
+    n = 1 << 28
+    x = inp.make_ghost_values(1 << 20, seed=3)
+    xd = torch.from_numpy(x).to(dev).repeat(n // x.size)
+    for nbits in (16, 12, 10):
+        sd = torch.empty(B.chfsi_bfp_stream_bytes(nbits, n), dtype=torch.uint8, device=dev)
+        yd = torch.empty_like(xd)
+        nbytes = 4.0 * n + sd.numel()
+        t_enc = timed(lambda: B.chfsi_bfp_encode(nbits, xd, sd))
+        t_dec = timed(lambda: B.chfsi_bfp_decode(nbits, sd, yd))
+        for nm, t in (("bfp_encode", t_enc), ("bfp_decode", t_dec)):
+            gbs = nbytes / (t * 1e-3) / 1e9
+            rows.append({"kernel": nm, "n_bits": nbits, "values": n, "ms": round(t, 4), "bound": "hbm", "achieved_GBs": round(gbs, 1),
+                         "peak_GBs": hbm_peak, "frac": round(gbs / hbm_peak, 4)})
+        del sd, yd
+    del xd
+    torch.cuda.empty_cache()
+
+    # ---- Rayleigh-Ritz pieces on configs[2]'s mesh rows (3.54M rows) x 256 vectors
+    cfg = inp.CONFIGS[2]
+    nv = 256
+    mesh = B.chfsi_mesh_create(cfg.ncell, cfg.L, cfg.p, cfg.kfrac, device)
+    try:
+        g = torch.Generator(device=dev); g.manual_seed(77)
+        Y = torch.empty((cfg.nnodes, 2, nv), dtype=torch.complex128, device=dev)
+        Yr = torch.view_as_real(Y)
+        for j0 in range(0, nv, 64):
+            Yr[:, :, j0:j0 + 64, :] = torch.rand((cfg.nnodes, 2, 64, 2), generator=g, device=dev, dtype=torch.float64) - 0.5
+        S = torch.empty((nv, nv), dtype=torch.complex128, device=dev)
+        nrows = 2 * cfg.nnodes
+        t = timed(lambda: B.chfsi_rr_project(mesh, Y, Y, S))
+        nt = (nv + 63) // 64
+        flops = 8.0 * nrows * 64 * 64 * (nt * (nt + 1) // 2)          # complex MAC = 8 flop; tiles on and above the diagonal
+        rows.append({"kernel": "rr_project (Y^H M Y, Hermitian)", "rows": nrows, "nvec": nv, "ms": round(t, 3), "bound": "alu",
+                     "achieved_TFs": round(flops / (t * 1e-3) / 1e12, 2), "peak_TFs": round(pipe["fp64_fma"], 2),
+                     "frac": round(flops / (t * 1e-3) / 1e12 / pipe["fp64_fma"], 4), "dtype": "f64"})
+        Q = torch.linalg.qr(torch.randn((nv, nv), dtype=torch.complex128, device=dev, generator=g))[0].contiguous()
+        Yo = torch.empty_like(Y)
+        wk = torch.empty(B.chfsi_rr_rotate_workspace_bytes(nv), dtype=torch.uint8, device=dev)
+        flops = 8.0 * nrows * nv * nv
+        for prec, nm, pk in ((B.FP32, "rr_rotate (FP64 diagonal + FP32 off-diagonal)", "fp32_fma"), (B.FP64, "rr_rotate (FP64)", "fp64_fma")):
+            t = timed(lambda: B.chfsi_rr_rotate(prec, Y, Q, Yo, wk), reps=2)
+            rows.append({"kernel": nm, "rows": nrows, "nvec": nv, "ms": round(t, 3), "bound": "alu",
+                         "achieved_TFs": round(flops / (t * 1e-3) / 1e12, 2), "peak_TFs": round(pipe[pk], 2),
+                         "frac": round(flops / (t * 1e-3) / 1e12 / pipe[pk], 4), "dtype": "f32 off-diagonal / f64 diagonal" if prec == B.FP32 else "f64"})
+    finally:
+        B.chfsi_mesh_destroy(mesh)
+        torch.cuda.empty_cache()
+    return rows
+
 # --------------------------------------------------------------------------------------------
 def run_e2e(torch, B, w, world, dist, barrier, n_steps):
     """The same filter through the C ABI with HOST buffers: every step uploads all of X from pinned host memory and
@@ -473,9 +539,11 @@ def run_ours(args, cfg):
         e2e = run_e2e(torch, B, w, world, dist, barrier, max(1, min(args.steps, 2 if big else 5)))
 
     w.close()
-    table = None
+    table, pipe, extra = None, None, None
     if rank == 0 and world == 1 and not args.no_table:
         table = all_configs_table(torch, B, local, peak)
+        pipe = B.chfsi_measure_pipe_peaks(local)
+        extra = extra_kernels(torch, B, local, peak, pipe)
 
     # ---- CPU oracle baseline on a bounded sample (rank 0, N = 1 only)
     cpu = None
@@ -498,6 +566,7 @@ def run_ours(args, cfg):
             "gpu_launches": int(launches), "clocks": clocks,
             "roofline_whole_filter": {"alg_bytes_per_unit": bpu, "frac_of_hbm_peak": value / world * bpu / (peak * 1e9)},
             "all_configs": table,
+            "pipe_peaks_TFs": pipe, "other_kernels": extra,
         }
         print(json.dumps(line))
     if dist is not None:
