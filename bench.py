@@ -356,6 +356,7 @@ def extra_kernels(torch, B, device, hbm_peak, pipe):
     cfg = inp.CONFIGS[2]
     nv = 256
     mesh = B.chfsi_mesh_create(cfg.ncell, cfg.L, cfg.p, cfg.kfrac, device)
+    B.chfsi_ham_set(mesh, None, None, None, None)
     try:
         g = torch.Generator(device=dev); g.manual_seed(77)
         Y = torch.empty((cfg.nnodes, 2, nv), dtype=torch.complex128, device=dev)

@@ -243,7 +243,7 @@ chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
         if (m->side) cudaStreamDestroy(m->side);
         for (cudaEvent_t e : m->stage_ev) if (e) cudaEventDestroy(e);
         if (m->h_stage) cudaFreeHost(m->h_stage);
-        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF);
+        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF); cudaFree(m->dMass);
         free_nonlocal(m->nl);
     }
     delete m;
@@ -381,6 +381,12 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
     free_nonlocal(m->nl);
     m->nl = nl;
     nlguard.p = nullptr;
+    if (!m->dMass) {     // node masses on the device (setup call: allocation is allowed here)
+        std::vector<double> mass((size_t)m->nnodes);
+        for (long long I = 0; I < m->nnodes; ++I) mass[(size_t)I] = node_mass(m, I);
+        CU(upload(&m->dMass, mass));
+    }
+    m->bare_laplacian = (V == nullptr && Bx == nullptr && By == nullptr && Bz == nullptr && natoms == 0);
     if (!m->h_stage) {   // pinned staging ring of the filter's coefficient program (setup call: allocation is allowed here)
         m->stage_slot_doubles = 4 + 9 * (size_t)(kDegreeCap + 2) + chfsi_mesh::kStageLambda;
         CU(cudaHostAlloc(reinterpret_cast<void**>(&m->h_stage), chfsi_mesh::kStageSlots * m->stage_slot_doubles * sizeof(double),

@@ -10,28 +10,13 @@
 
 namespace chfsi {
 
-struct MassArgs {
-    int use;                    // 0: w = 1
-    int p, n1x, n1y;
-    double m1[3][kMaxN];        // 1-D mass factors at the cell-local index (face nodes doubled)
-};
-
-__device__ __forceinline__ double row_mass(const MassArgs& ma, long long row) {
-    if (!ma.use) return 1.0;
-    const long long I = row >> 1;
-    const int ix = (int)(I % ma.n1x);
-    const long long r2 = I / ma.n1x;
-    const int iy = (int)(r2 % ma.n1y), iz = (int)(r2 / ma.n1y);
-    return ma.m1[0][ix % ma.p] * ma.m1[1][iy % ma.p] * ma.m1[2][iz % ma.p];
-}
-
 // ---- S += A^H diag(w) B over this CTA's slab of rows.  Tile 64 x 64 complex, 16 x 16 threads, 4 x 4 outputs per thread
 //      (i = ty + 16 a, j = tx + 16 b); K-slabs of 8 rows, double buffered through registers.
 constexpr int PT = 64, PK = 8;
 
 __global__ void __launch_bounds__(256) rr_project_kernel(const double2* __restrict__ A, long long lda, const double2* __restrict__ B,
                                                          long long ldb, long long nrows, int nvec, long long rows_per_cta,
-                                                         const __grid_constant__ MassArgs ma, int hermitian, double2* __restrict__ S) {
+                                                         const double* __restrict__ mass, int hermitian, double2* __restrict__ S) {
     const int ti = blockIdx.y, tj = blockIdx.x;
     if (hermitian && tj < ti) return;                       // the lower triangle is mirrored afterwards
     __shared__ double2 As[PK][PT], Bs[PK][PT];
@@ -54,7 +39,7 @@ __global__ void __launch_bounds__(256) rr_project_kernel(const double2* __restri
             const int ci = ti * PT + lc, cj = tj * PT + lc;
             ra[h] = (ok && ci < nvec) ? __ldg(A + r * lda + ci) : make_double2(0.0, 0.0);
             double2 bv = (ok && cj < nvec) ? __ldg(B + r * ldb + cj) : make_double2(0.0, 0.0);
-            const double w = ok ? row_mass(ma, r) : 0.0;
+            const double w = ok ? (mass ? __ldg(mass + (r >> 1)) : 1.0) : 0.0;      // row 2 I + alpha carries m_I
             rb[h] = make_double2(bv.x * w, bv.y * w);
         }
     };
@@ -131,20 +116,33 @@ __global__ void __launch_bounds__(256) rr_rotate_kernel(const double2* __restric
     for (int a = 0; a < RA; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b) { cre[a][b] = 0; cim[a][b] = 0; }
-    for (int i0 = 0; i0 < nvec; i0 += KT) {
-        // Y tile: RT rows x 8 columns (a row's 8 columns are 128 contiguous bytes); converted to TC on the way in
-        for (int e = tid; e < RT * KT; e += 256) {
-            const int rr = e / KT, kk = e % KT;
+    // loader: the Y tile is RT rows x 8 columns (a row's 8 columns are 128 contiguous bytes), the Q tile 8 x 64; both are
+    // fetched into registers one slab ahead of the arithmetic and converted to TC on the way
+    constexpr int NY = RT * KT / 256, NQ = KT * PT / 256;
+    TC2 ry[NY], rq[NQ];
+    auto fetch = [&](int i0) {
+#pragma unroll
+        for (int u = 0; u < NY; ++u) {
+            const int e = tid + 256 * u, rr = e / KT, kk = e % KT;
             const long long r = rbase + rr;
             const double2 v = (r < nrows && i0 + kk < nvec) ? __ldg(Y + r * ldy + i0 + kk) : make_double2(0.0, 0.0);
-            Ys[kk][rr].x = (TC)v.x; Ys[kk][rr].y = (TC)v.y;
+            ry[u].x = (TC)v.x; ry[u].y = (TC)v.y;
         }
-        for (int e = tid; e < KT * PT; e += 256) {
-            const int kk = e / PT, jj = e % PT;
+#pragma unroll
+        for (int u = 0; u < NQ; ++u) {
+            const int e = tid + 256 * u, kk = e / PT, jj = e % PT;
             TC2 z; z.x = 0; z.y = 0;
-            Qs[kk][jj] = (i0 + kk < nvec && jbase + jj < nvec) ? Qo[(long long)(i0 + kk) * nvec + jbase + jj] : z;
+            rq[u] = (i0 + kk < nvec && jbase + jj < nvec) ? Qo[(long long)(i0 + kk) * nvec + jbase + jj] : z;
         }
+    };
+    fetch(0);
+    for (int i0 = 0; i0 < nvec; i0 += KT) {
+#pragma unroll
+        for (int u = 0; u < NY; ++u) { const int e = tid + 256 * u; Ys[e % KT][e / KT] = ry[u]; }
+#pragma unroll
+        for (int u = 0; u < NQ; ++u) { const int e = tid + 256 * u; Qs[e / PT][e % PT] = rq[u]; }
         __syncthreads();
+        if (i0 + KT < nvec) fetch(i0 + KT);
 #pragma unroll
         for (int k = 0; k < KT; ++k) {
             TC2 y[RA], q[4];
@@ -197,13 +195,12 @@ chfsi_status chfsi_rr_project(const chfsi_mesh* mesh, long long nrows, int nvec,
     if (!A || !B || !S) return rr_fail(CHFSI_EINVAL, "rr_project: NULL device pointer");
     if (lda < nvec || ldb < nvec) return rr_fail(CHFSI_EINVAL, "rr_project: leading dimension < nvec");
     if (((uintptr_t)A & 15) || ((uintptr_t)B & 15) || ((uintptr_t)S & 15)) return rr_fail(CHFSI_EINVAL, "rr_project: pointers must be 16-byte aligned");
-    MassArgs ma{};
+    const double* mass = nullptr;
     if (use_mass) {
         if (!mesh) return rr_fail(CHFSI_EINVAL, "rr_project: the mass weighting needs a mesh");
+        if (!mesh->dMass) return rr_fail(CHFSI_ESTATE, "rr_project: chfsi_ham_set has not been called (it builds the device mass)");
         if (nrows != 2 * mesh->nnodes) return rr_fail(CHFSI_EINVAL, "rr_project: with the mass weighting nrows must be 2 * nnodes");
-        ma.use = 1; ma.p = mesh->p; ma.n1x = mesh->mc.n1[0]; ma.n1y = mesh->mc.n1[1];
-        for (int d = 0; d < 3; ++d)
-            for (int a = 0; a < kMaxN; ++a) ma.m1[d][a] = mesh->mc.m1[d][a];
+        mass = mesh->dMass;
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     chfsi_status rc = rr_cuda(cudaMemsetAsync(S, 0, (size_t)nvec * nvec * 16, st), "rr_project memset");
@@ -219,7 +216,7 @@ chfsi_status chfsi_rr_project(const chfsi_mesh* mesh, long long nrows, int nvec,
     nz = nrows > 0 ? (nrows + rows_per - 1) / rows_per : 0;
     if (nz > 0) {
         rr_project_kernel<<<dim3(nt, nt, (unsigned)nz), 256, 0, st>>>(static_cast<const double2*>(A), lda, static_cast<const double2*>(B), ldb,
-                                                                      nrows, nvec, rows_per, ma, hermitian ? 1 : 0, static_cast<double2*>(S));
+                                                                      nrows, nvec, rows_per, mass, hermitian ? 1 : 0, static_cast<double2*>(S));
         rc = rr_cuda(cudaGetLastError(), "rr_project");
         if (rc != CHFSI_OK) return rc;
         count_launch();

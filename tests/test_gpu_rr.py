@@ -114,6 +114,7 @@ def test_project_full_size_block_properties(env, ro):
     torch, fo, B = env
     cfg = inp.CONFIGS[1]
     mesh = B.chfsi_mesh_create(cfg.ncell, cfg.L, cfg.p, cfg.kfrac, 0)
+    B.chfsi_ham_set(mesh, None, None, None, None)                       # builds the device mass (bare Laplacian)
     try:
         cols = [0, 1, 63, 64, 127]
         Yc = inp.make_vectors(cfg.nnodes, cols)
