@@ -215,6 +215,30 @@ chfsi_status chfsi_rr_rotate_workspace_bytes(int nvec, size_t* bytes);
 chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q,
                              void* Yout, long long ldo, void* work, size_t work_bytes, void* cuda_stream);
 
+/* ---- matrix-free Poisson solve (eq. 5-6; Kx kernel and Algorithm 2) -----
+ * Solves K x = f for the stiffness matrix K of -laplace on the handle's periodic mesh (GLL quadrature: K = 2 x the kinetic
+ * part of H; reading P2), batched: a spinor-layout block [2 M rows][ld complex128] holds 4 nvec independent real
+ * right-hand sides, column id cid = (s nvec + v) 2 + ri for spin row s, vector v, real / imaginary part ri (eq. 6 has one
+ * problem per atom).  The handle's Hamiltonian must be the bare Laplacian: chfsi_ham_set(mesh, NULL, NULL, NULL, NULL, 0, ...),
+ * kfrac = 0 and at least two cells per direction (ESTATE / EINVAL otherwise).  K is singular (constants): every column of f
+ * must sum to zero; x starts at 0 and is returned with zero mass-weighted mean.
+ * chfsi_poisson_kdiag: diag(K), host output, M doubles (the Jacobi scaling; the caller estimates the spectral bounds of
+ *   K_diag^-1 K with it, "a short Lanczos run on the scaled operator").
+ * chfsi_poisson_apply_K: W = K U (the Kx kernel: gather + sum-factorised contractions + assembly in one launch).
+ * chfsi_poisson_pcg: Algorithm 2 with the degree-`cheb_degree` Chebyshev-Jacobi preconditioner on [lmin, lmax] (cheb_degree - 1
+ *   extra Kx per iteration); stops a column when sqrt(|r|^2) < tol (absolute) or after maxit iterations.  The scalars stay on
+ *   the device; the host reads the number of unconverged columns every `check_every` iterations (0: never -- the call then
+ *   runs maxit iterations without synchronising).  iters_host / resnorm_host (host, 4 nvec each, may be NULL; reading them
+ *   synchronises): iterations taken and final residual norm per column.  work: chfsi_poisson_workspace_bytes, 256-byte aligned.
+ *   FP64 throughout. */
+chfsi_status chfsi_poisson_kdiag(const chfsi_mesh* mesh, double* kdiag_host);
+chfsi_status chfsi_poisson_apply_K(const chfsi_mesh* mesh, int nvec, const void* U, long long ldu, void* W, long long ldw,
+                                   void* cuda_stream);
+chfsi_status chfsi_poisson_workspace_bytes(const chfsi_mesh* mesh, int nvec, size_t* bytes);
+chfsi_status chfsi_poisson_pcg(const chfsi_mesh* mesh, int nvec, const void* F, long long ldf, void* X, long long ldx,
+                               int cheb_degree, double lmin, double lmax, double tol, int maxit, int check_every,
+                               void* work, size_t work_bytes, int* iters_host, double* resnorm_host, void* cuda_stream);
+
 /* ---- measurement aid: issue-rate peaks of the FMA and mma.sync pipes ------------------------------
  * Runs four register-resident micro-kernels on `device` (one 512-thread CTA per SM, a few milliseconds each, synchronises)
  * and returns TFLOP/s (2 flop per FMA) in tflops[0..3]: FP64 FMA, FP32 FMA, mma.m8n8k4.f64, mma.m16n8k8.tf32.  bench.py

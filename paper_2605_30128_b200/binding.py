@@ -27,6 +27,7 @@ EXPORTS = [
     "chfsi_bfp_stream_bytes", "chfsi_bfp_encode", "chfsi_bfp_decode", "chfsi_bfp_gather_encode",
     "chfsi_bfp_decode_scatter_add",
     "chfsi_rr_project", "chfsi_rr_rotate_workspace_bytes", "chfsi_rr_rotate", "chfsi_measure_pipe_peaks",
+    "chfsi_poisson_kdiag", "chfsi_poisson_apply_K", "chfsi_poisson_workspace_bytes", "chfsi_poisson_pcg",
     "chfsi_last_launch_count", "chfsi_last_error", "chfsi_version",
 ]
 
@@ -72,6 +73,11 @@ def lib() -> C.CDLL:
     L.chfsi_rr_rotate_workspace_bytes.argtypes = [C.c_int, C.POINTER(C.c_size_t)]
     L.chfsi_rr_rotate.argtypes = [C.c_int, C.c_longlong, C.c_int, vp, C.c_longlong, vp, vp, C.c_longlong, vp, C.c_size_t, vp]
     L.chfsi_measure_pipe_peaks.argtypes = [C.c_int, dp]
+    L.chfsi_poisson_kdiag.argtypes = [vp, dp]
+    L.chfsi_poisson_apply_K.argtypes = [vp, C.c_int, vp, C.c_longlong, vp, C.c_longlong, vp]
+    L.chfsi_poisson_workspace_bytes.argtypes = [vp, C.c_int, C.POINTER(C.c_size_t)]
+    L.chfsi_poisson_pcg.argtypes = [vp, C.c_int, vp, C.c_longlong, vp, C.c_longlong, C.c_int, C.c_double, C.c_double, C.c_double,
+                                    C.c_int, C.c_int, vp, C.c_size_t, ip, dp, vp]
     for name in EXPORTS:
         if name not in ("chfsi_last_launch_count", "chfsi_last_error", "chfsi_version"):
             getattr(L, name).restype = C.c_int
@@ -266,3 +272,34 @@ def chfsi_measure_pipe_peaks(device=0) -> dict:
     out = (C.c_double * 4)()
     _check(lib().chfsi_measure_pipe_peaks(int(device), out))
     return {"fp64_fma": out[0], "fp32_fma": out[1], "fp64_mma": out[2], "tf32_mma": out[3]}
+
+
+# ---- Poisson solve ----------------------------------------------------------------
+def chfsi_poisson_kdiag(mesh) -> np.ndarray:
+    kd = np.empty(chfsi_mesh_num_nodes(mesh), dtype=np.float64)
+    _check(lib().chfsi_poisson_kdiag(mesh, _dptr(kd)))
+    return kd
+
+
+def chfsi_poisson_apply_K(mesh, U, W, stream=None):
+    """U, W: torch complex128 CUDA tensors [M, 2, ld] (4 nvec independent real columns)."""
+    _check(lib().chfsi_poisson_apply_K(mesh, U.shape[-1], _ptr(U), U.stride(-2), _ptr(W), W.stride(-2), _stream(stream)))
+
+
+def chfsi_poisson_workspace_bytes(mesh, nvec) -> int:
+    b = C.c_size_t()
+    _check(lib().chfsi_poisson_workspace_bytes(mesh, int(nvec), C.byref(b)))
+    return b.value
+
+
+def chfsi_poisson_pcg(mesh, F, X, cheb_degree, lmin, lmax, tol, maxit, work, check_every=10, stream=None, want_stats=True):
+    """Returns (iterations, residual norms) per real column [2, nvec, 2] = (spin, vector, re/im) when want_stats."""
+    nvec = F.shape[-1]
+    it = np.zeros(4 * nvec, dtype=np.int32) if want_stats else None
+    rn = np.zeros(4 * nvec, dtype=np.float64) if want_stats else None
+    _check(lib().chfsi_poisson_pcg(mesh, nvec, _ptr(F), F.stride(-2), _ptr(X), X.stride(-2), int(cheb_degree), float(lmin),
+                                   float(lmax), float(tol), int(maxit), int(check_every), _ptr(work), work.numel(),
+                                   None if it is None else it.ctypes.data_as(C.POINTER(C.c_int)), _dptr(rn), _stream(stream)))
+    if not want_stats:
+        return None, None
+    return it.reshape(2, nvec, 2), rn.reshape(2, nvec, 2)

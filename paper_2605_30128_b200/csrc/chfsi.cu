@@ -243,7 +243,7 @@ chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
         if (m->side) cudaStreamDestroy(m->side);
         for (cudaEvent_t e : m->stage_ev) if (e) cudaEventDestroy(e);
         if (m->h_stage) cudaFreeHost(m->h_stage);
-        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF); cudaFree(m->dMass);
+        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF); cudaFree(m->dMass); cudaFree(m->dKdiag);
         free_nonlocal(m->nl);
     }
     delete m;
@@ -385,6 +385,29 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
         std::vector<double> mass((size_t)m->nnodes);
         for (long long I = 0; I < m->nnodes; ++I) mass[(size_t)I] = node_mass(m, I);
         CU(upload(&m->dMass, mass));
+    }
+    if (!m->dKdiag && m->nc[0] > 1 && m->nc[1] > 1 && m->nc[2] > 1) {
+        // diag(K), K = 2 x (kinetic part): the assembled diagonal of a separable cell matrix factorises into assembled 1-D
+        // diagonals: diag(K/2)_I = kx[ix] wy[iy] wz[iz] + wx[ix] ky[iy] wz[iz] + wx[ix] wy[iy] kz[iz]
+        const int p = m->p;
+        std::vector<double> k1[3], w1[3];
+        for (int d = 0; d < 3; ++d) {
+            const int n1 = m->mc.n1[d];
+            k1[d].assign(n1, 0.0); w1[d].assign(n1, 0.0);
+            for (int g = 0; g < n1; ++g) {
+                const int a = g % p;
+                k1[d][g] = m->mc.Kd[d][a][a] + (a == 0 ? m->mc.Kd[d][p][p] : 0.0);
+                w1[d][g] = m->mc.w[a] + (a == 0 ? m->mc.w[p] : 0.0);
+            }
+        }
+        std::vector<double> kd((size_t)m->nnodes);
+        const int nx = m->mc.n1[0], ny = m->mc.n1[1], nz = m->mc.n1[2];
+        for (int iz = 0; iz < nz; ++iz)
+            for (int iy = 0; iy < ny; ++iy)
+                for (int ix = 0; ix < nx; ++ix)
+                    kd[((size_t)iz * ny + iy) * nx + ix] = 2.0 * (k1[0][ix] * w1[1][iy] * w1[2][iz] + w1[0][ix] * k1[1][iy] * w1[2][iz] +
+                                                                  w1[0][ix] * w1[1][iy] * k1[2][iz]);
+        CU(upload(&m->dKdiag, kd));
     }
     m->bare_laplacian = (V == nullptr && Bx == nullptr && By == nullptr && Bz == nullptr && natoms == 0);
     if (!m->h_stage) {   // pinned staging ring of the filter's coefficient program (setup call: allocation is allowed here)

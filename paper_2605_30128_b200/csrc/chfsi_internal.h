@@ -123,6 +123,7 @@ struct chfsi_mesh {
     double* dBz = nullptr;
     double* dF = nullptr;               // packed fields [M][4] = V+Bz, V-Bz, Bx, By (march kernel)
     double* dMass = nullptr;            // node masses m_I [M] (Rayleigh-Ritz projection, Poisson solver); built in chfsi_ham_set
+    double* dKdiag = nullptr;           // diag(K) of the stiffness matrix K = 2 x kinetic part [M] (Poisson preconditioner); built in chfsi_ham_set
     bool bare_laplacian = false;        // the Hamiltonian set last has no local fields and no projectors (Poisson handle)
     chfsi::NonlocalDev nl;
     // profiling aid (chfsi_profile_enable / chfsi_profile_read)
