@@ -383,6 +383,53 @@ def extra_kernels(torch, B, device, hbm_peak, pipe):
     finally:
         B.chfsi_mesh_destroy(mesh)
         torch.cuda.empty_cache()
+
+    # ---- Poisson: the Kx kernel and the batched PCG (Algorithm 2) on configs[3]'s mesh (96^3 nodes, p = 8), 64 right-hand sides
+    cfg = inp.CONFIGS[3]
+    nv = 16                                                   # 4 nv = 64 real columns
+    mesh = B.chfsi_mesh_create(cfg.ncell, cfg.L, cfg.p, (0.0, 0.0, 0.0), device)
+    B.chfsi_ham_set(mesh, None, None, None, None)
+    try:
+        g = torch.Generator(device=dev); g.manual_seed(78)
+        U = torch.empty((cfg.nnodes, 2, nv), dtype=torch.complex128, device=dev)
+        torch.view_as_real(U)[...] = torch.rand((cfg.nnodes, 2, nv, 2), generator=g, device=dev, dtype=torch.float64) - 0.5
+        W = torch.empty_like(U)
+        t = timed(lambda: B.chfsi_poisson_apply_K(mesh, U, W), reps=5)
+        dofs = cfg.nnodes * 4.0 * nv
+        nbytes = dofs * 32.0                                  # u read 8 B, w zero-filled 8 B, w read-modify-written 16 B
+        rows.append({"kernel": "poisson Kx (memset + cell kernel)", "nodes": cfg.nnodes, "real_columns": 4 * nv, "ms": round(t, 4),
+                     "dof_per_s": float(f"{dofs / (t * 1e-3):.4g}"), "bound": "hbm", "achieved_GBs": round(nbytes / (t * 1e-3) / 1e9, 1),
+                     "peak_GBs": hbm_peak, "frac": round(nbytes / (t * 1e-3) / 1e9 / hbm_peak, 4), "dtype": "f64"})
+        mass = torch.from_numpy(B.chfsi_mesh_mass(mesh)).to(dev)
+        F = U * mass[:, None, None]
+        Fr = torch.view_as_real(F)
+        Fr -= Fr.mean(dim=0, keepdim=True)                    # neutral right-hand sides
+        kd = torch.from_numpy(B.chfsi_poisson_kdiag(mesh)).to(dev)
+        # upper spectral bound of K_diag^-1 K: ten power steps in the K_diag inner product (harness side), plus 10 %
+        V1 = torch.zeros((cfg.nnodes, 2, 1), dtype=torch.complex128, device=dev)
+        W1 = torch.empty_like(V1)
+        xv = torch.rand(cfg.nnodes, generator=g, device=dev, dtype=torch.float64) - 0.5
+        lam = 1.0
+        for _ in range(10):
+            V1[:, 0, 0] = xv
+            B.chfsi_poisson_apply_K(mesh, V1, W1)
+            yv = W1[:, 0, 0].real / kd
+            lam = float((kd * xv * yv).sum() / (kd * xv * xv).sum())
+            xv = yv / yv.abs().max()
+        lmax = 1.1 * lam
+        X = torch.empty_like(F)
+        wk = torch.empty(B.chfsi_poisson_workspace_bytes(mesh, nv), dtype=torch.uint8, device=dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        it, res = B.chfsi_poisson_pcg(mesh, F, X, 5, lmax / 30.0, lmax, 1e-10, 400, wk, check_every=10)
+        e1.record(); torch.cuda.synchronize()
+        tp = e0.elapsed_time(e1)
+        rows.append({"kernel": "poisson PCG (Alg. 2, degree-5 Chebyshev-Jacobi, tol 1e-10)", "nodes": cfg.nnodes, "real_columns": 4 * nv,
+                     "ms": round(tp, 2), "iterations_max": int(it.max()), "residual_max": float(res.max()),
+                     "kx_dof_per_s": float(f"{dofs * 5 * int(it.max()) / (tp * 1e-3):.4g}"), "dtype": "f64"})
+    finally:
+        B.chfsi_mesh_destroy(mesh)
+        torch.cuda.empty_cache()
     return rows
 
 # --------------------------------------------------------------------------------------------
