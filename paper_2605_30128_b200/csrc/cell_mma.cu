@@ -66,7 +66,10 @@ struct MmaCfg {
     static constexpr int C = 2 * MROWS, NV = C / 4;          // real batch columns of the CTA: both spin components
     static constexpr int NR = MROWS / 8, KH = KSTEP / 4;     // fragment rows g + 8r, fragment k-halves
     static constexpr int KS = (n + KSTEP - 1) / KSTEP, NT = (n + 7) / 8;
-    static constexpr int NCW = n;                            // consumer warps: index q in 0..p; a warp runs both m-tiles
+    // m-tiles per consumer warp.  2: one warp per index q running both halves of the CTA's vectors (9 warps at p = 8, ~140
+    // registers, 2.56e9 warp instructions per configs[3] launch, 6.3 ms); 1: one warp per (q, m-tile) (18 warps, 96 registers).
+    static constexpr int MTW = P >= 8 ? 2 : 1;       // measured: configs[3] (p = 8) 6.4 vs 6.9 ms, configs[4] (p = 6) 7.5 vs 7.2 ms
+    static constexpr int NCW = n * (2 / MTW);                // consumer warps
     static constexpr int THREADS = (NCW + 1) * 32;
     static constexpr int ESZ = (int)sizeof(T);
     static_assert(C * ESZ == 128, "one node of the CTA's columns is one 128-byte row");
@@ -167,25 +170,26 @@ struct Acc {
     }
 };
 
-// acc[mt] += K applied along the line whose 8-byte units at element kmap(ks, h, t) are ld(ks, h, u[2]) for the two m-tiles:
+// acc[mt] += K applied along the line whose 8-byte units at element kmap(ks, h, t) are ld(ks, h, u[MTW]) for the warp's m-tiles:
 // a double (FP64, fragment row g) or a float2 = (fragment row g, fragment row g + 8) (TF32)
 template <int P, int MODE, typename LD>
-__device__ __forceinline__ void contract(Acc<P, MODE> (&acc)[2], const BFrags<P, MODE>& bf, int t, LD ld) {
+__device__ __forceinline__ void contract(Acc<P, MODE> (&acc)[MmaCfg<P, MODE>::MTW], const BFrags<P, MODE>& bf, int t, LD ld) {
     using Cfg = MmaCfg<P, MODE>;
     using T = typename Cfg::T;
     using U = typename std::conditional<MODE == MM_F64, double, float2>::type;
 #pragma unroll
     for (int ks = 0; ks < Cfg::KS; ++ks) {
-        T a[2][Cfg::NR][Cfg::KH];
+        constexpr int MTW = Cfg::MTW;
+        T a[MTW][Cfg::NR][Cfg::KH];
 #pragma unroll
         for (int h = 0; h < Cfg::KH; ++h) {
             // the last k-step is only partly populated: lanes beyond the line contribute zeros
             const bool all = kmap<MODE>(ks, h, 3) < Cfg::n;
             const bool ok = all || kmap<MODE>(ks, h, t) < Cfg::n;
-            U u[2];
+            U u[MTW];
             if (ok) ld(ks, h, u);
 #pragma unroll
-            for (int mt = 0; mt < 2; ++mt) {
+            for (int mt = 0; mt < MTW; ++mt) {
                 if constexpr (MODE == MM_F64) {
                     a[mt][0][h] = ok ? u[mt] : 0.0;
                 } else {
@@ -194,7 +198,7 @@ __device__ __forceinline__ void contract(Acc<P, MODE> (&acc)[2], const BFrags<P,
             }
         }
 #pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
+        for (int mt = 0; mt < MTW; ++mt) {
             if constexpr (MODE == MM_F64) {
 #pragma unroll
                 for (int nt = 0; nt < Cfg::NT; ++nt) mma_f64(acc[mt].d[nt], a[mt][0][0], bf.hi[ks][nt][0]);
@@ -229,7 +233,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
     constexpr bool F64 = MODE == MM_F64;
     using U = typename std::conditional<F64, double, float2>::type;      // the thread's 8-byte unit of a node row
     constexpr int n = Cfg::n, C = Cfg::C, S = Cfg::S, RS = Cfg::RS, XPU = Cfg::XPU, NR = Cfg::NR, NT = Cfg::NT;
-    constexpr int ESZ = Cfg::ESZ, KS = Cfg::KS, KH = Cfg::KH;
+    constexpr int ESZ = Cfg::ESZ, KS = Cfg::KS, KH = Cfg::KH, MTW = Cfg::MTW;
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t full_in[S], empty_in[S], full_r[RS], empty_r[RS];
     // the swizzle is a function of shared-memory address bits: work from a 1024-byte aligned base
@@ -305,25 +309,25 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
     // ================================ consumers ================================
     // warp = index q in 0..p: row j of the X and Z tasks, x-position i of the Y task; it runs both m-tiles (mt = 0, 1: the two
     // halves of the CTA's vectors), whose units sit 32 bytes apart in a node row
-    const int q = warp;
+    const int q = warp / (2 / MTW), mt0 = warp % (2 / MTW);
     const int g = lane >> 2, t4 = lane & 3;
     // the thread's 8-byte unit inside a node's 128-byte row: bit 3 = g & 1, spin (bit 6) = (g >> 1) & 1, chunk = 2 mt + (g >> 2)
     const int spin = (g >> 1) & 1;
-    const uint32_t fb0 = (uint32_t)(spin * 64 + (g >> 2) * 16 + (g & 1) * 8);       // m-tile 0; m-tile 1 is 32 bytes on
+    const uint32_t fb0 = (uint32_t)(spin * 64 + (2 * mt0 + (g >> 2)) * 16 + (g & 1) * 8);   // first m-tile of the warp; the next is 32 bytes on
     const int upos = (int)(fb0 >> 3);             // unit index inside the node (XR); m-tile 1: + 4
     // TF32: unit = complex64 of vector vl; FP64: unit = the re (ri = 0) or im (ri = 1) part of vector vl; m-tile 1: vl + VSTEP
     constexpr int VSTEP = F64 ? 2 : 4;
-    const int vl = F64 ? (g >> 2) : 2 * (g >> 2) + (g & 1);
+    const int vl = (F64 ? (g >> 2) : 2 * (g >> 2) + (g & 1)) + VSTEP * mt0;
     const int ri = F64 ? (g & 1) : 0;
     const double sgs = spin == 0 ? 1.0 : -1.0;    // sign of B_y in (B_x -+ i B_y)
     const int NTH = Cfg::NCW * 32;
     BFrags<P, MODE> bf;
     bf.init(sc, g, t4);
     const int v = chunk * Cfg::NV + vl;
-    bool vok[2];
-    double cin[2], cR[2];
+    bool vok[MTW];
+    double cin[MTW], cR[MTW];
 #pragma unroll
-    for (int mt = 0; mt < 2; ++mt) {
+    for (int mt = 0; mt < MTW; ++mt) {
         vok[mt] = FULLV || v + VSTEP * mt < ar.nvec;
         cin[mt] = (vok[mt] && ar.cin) ? __ldg(ar.cin + v + VSTEP * mt) : 0.0;
         cR[mt] = (vok[mt] && ar.cR && ar.useR) ? __ldg(ar.cR + v + VSTEP * mt) : 0.0;
@@ -356,10 +360,10 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
         }
     auto ldu = [&](uint32_t lin) { return *reinterpret_cast<const U*>(smem + swz64(lin)); };
     // the units of both m-tiles at (m-tile 0) offset lin: bit 5 of lin is clear, so "+ 32" commutes with the swizzle as "^ 32"
-    auto ldu2 = [&](uint32_t lin, U (&u)[2]) {
+    auto ldu2 = [&](uint32_t lin, U (&u)[MTW]) {
         const uint32_t a = swz64(lin);
         u[0] = *reinterpret_cast<const U*>(smem + a);
-        u[1] = *reinterpret_cast<const U*>(smem + (a ^ 32u));
+        if constexpr (MTW == 2) u[1] = *reinterpret_cast<const U*>(smem + (a ^ 32u));
     };
 
     // a complex output value held as d[0] = re, d[1] = im (TF32) or as the component ri of it (FP64, partner in lane ^ 4)
@@ -399,7 +403,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                     if (fx) { const double u = pr * ar.ph_re[0] - pi * ar.ph_im[0]; pi = pr * ar.ph_im[0] + pi * ar.ph_re[0]; pr = u; }
                     const uint32_t ea = swz64(sb + (uint32_t)(q * n + (valid ? i : 0)) * 128u + fb0);
 #pragma unroll
-                    for (int mt = 0; mt < 2; ++mt) {
+                    for (int mt = 0; mt < MTW; ++mt) {
                         U* e = reinterpret_cast<U*>(smem + (ea ^ (mt ? 32u : 0u)));
                         if constexpr (F64) {
                             const double val = valid ? *e : 0.0;
@@ -419,9 +423,10 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 __syncwarp();
             }
         }
-        Acc<P, MODE> acc[2];
-        acc[0].zero(); acc[1].zero();
-        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[2]) { ldu2(sb + xa[ks][h], u); });
+        Acc<P, MODE> acc[MTW];
+#pragma unroll
+        for (int mt = 0; mt < MTW; ++mt) acc[mt].zero();
+        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[MTW]) { ldu2(sb + xa[ks][h], u); });
         U* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / 8) + (q * n) * XPU + upos;
         const bool s5on = up && q < P;
         if (s5on) mbar_wait(&full_r[rsl], rpar);
@@ -436,9 +441,9 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 const bool live = nt * 8 + 6 + e < n || xo < n;          // compile-time true for fully populated n-tiles
                 const int xoc = live ? xo : 0;
                 const bool own_node = s5on && live && (nt * 8 + 6 + e < P || xoc < P);
-                Val val[2];
+                Val val[MTW];
 #pragma unroll
-                for (int mt = 0; mt < 2; ++mt) {
+                for (int mt = 0; mt < MTW; ++mt) {
                     val[mt].a = sXWY * acc[mt].d[nt][0][e];
                     val[mt].b = NR == 2 ? sXWY * acc[mt].d[nt][NR - 1][e] : (T)0;
                 }
@@ -447,16 +452,16 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                     // z-weight because the Y task multiplies the whole XR entry by it
                     const double fd = Fs[xoc * 4 + spin], bx = Fs[xoc * 4 + 2], by = sgs * Fs[xoc * 4 + 3];
                     const uint32_t lin = sb + (uint32_t)(q * n + xoc) * 128u + fb0;
-                    U me[2], ot[2];
+                    U me[MTW], ot[MTW];
                     ldu2(lin, me);
                     ldu2(lin ^ 64u, ot);
                     if constexpr (F64) {
                         // own component ri of spin s; the other spin's same (ot) and other (of) component
-                        U of[2];
+                        U of[MTW];
                         ldu2(lin ^ 72u, of);
                         const uint32_t rs0 = swz64(rb + (uint32_t)(q * P + xoc) * 128u + fb0);
 #pragma unroll
-                        for (int mt = 0; mt < 2; ++mt) {
+                        for (int mt = 0; mt < MTW; ++mt) {
                             // s = 0: (B_x - i B_y) u' ; s = 1: (B_x + i B_y) u' ; re: B_x c + sgs B_y d ; im: B_x d - sgs B_y c
                             const double pot = fma(fd, me[mt], fma(bx, ot[mt], (ri ? -by : by) * of[mt]));
                             double s5 = fma(cin[mt], me[mt], sc.cHp * pot);
@@ -470,7 +475,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                         // FP32 arithmetic ("pointwise terms stay FP32", A7); the R-term is formed in FP64 and rounded once
                         const float fdf = (float)fd, bxf = (float)bx, byf = (float)by, chp = (float)sc.cHp;
 #pragma unroll
-                        for (int mt = 0; mt < 2; ++mt) {
+                        for (int mt = 0; mt < MTW; ++mt) {
                             const float a = me[mt].x, b = me[mt].y, c = ot[mt].x, d = ot[mt].y;
                             const float pre = fmaf(fdf, a, fmaf(bxf, c, byf * d)), pim = fmaf(fdf, b, fmaf(bxf, d, -byf * c));
                             float sre = fmaf((float)cin[mt], a, chp * pre), sim = fmaf((float)cin[mt], b, chp * pim);
@@ -485,7 +490,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                 }
                 if (live) {
 #pragma unroll
-                    for (int mt = 0; mt < 2; ++mt) {
+                    for (int mt = 0; mt < MTW; ++mt) {
                         if constexpr (F64) XR[xoc * XPU + 4 * mt] = val[mt].a;
                         else XR[xoc * XPU + 4 * mt] = make_float2(val[mt].a, val[mt].b);
                     }
@@ -499,9 +504,10 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
 
     // ---- Y task of plane tp: y-contraction at x-position q, + XR (x part and S5), times the plane's z-weight -> RED to out
     auto ytask = [&](int tp, uint32_t sb, T wz) {
-        Acc<P, MODE> acc[2];
-        acc[0].zero(); acc[1].zero();
-        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[2]) { ldu2(sb + ya[ks][h], u); });
+        Acc<P, MODE> acc[MTW];
+#pragma unroll
+        for (int mt = 0; mt < MTW; ++mt) acc[mt].zero();
+        contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[MTW]) { ldu2(sb + ya[ks][h], u); });
         const U* XR = XRb + (size_t)(tp & 1) * (Cfg::XR_BYTES / 8) + q * XPU + upos;
         const bool zwrap = (g0 + tp) == ar.n1[2];
         const bool zp = HASPH && zwrap && ar.phd[2];
@@ -526,7 +532,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                     const int yoc = live ? yo : 0;
                     const long long yq = nt == 0 ? (e == 0 ? yq0 : yq1) : (e == 0 ? yq8 : yq9);
 #pragma unroll
-                    for (int mt = 0; mt < 2; ++mt) {
+                    for (int mt = 0; mt < MTW; ++mt) {
                         const U xr = XR[(yoc * n) * XPU + 4 * mt];
                         Val val;
                         if constexpr (F64) { val.a = wz * fma(sYWX, acc[mt].d[nt][0][e], xr); val.b = 0; }
@@ -561,10 +567,11 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
         const long long zq9 = zoff(g0 + tb + (9 + 2 * t4 < n ? 9 + 2 * t4 : 0)) + zrow;
 #pragma unroll 1
         for (int i = 0; i < n; ++i) {
-            Acc<P, MODE> acc[2];
-            acc[0].zero(); acc[1].zero();
+            Acc<P, MODE> acc[MTW];
+#pragma unroll
+            for (int mt = 0; mt < MTW; ++mt) acc[mt].zero();
             const uint32_t no = (uint32_t)i * 128u;
-            contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[2]) { ldu2(zb[ks][h] + no, u); });
+            contract<P, MODE>(acc, bf, t4, [&](int ks, int h, U (&u)[MTW]) { ldu2(zb[ks][h] + no, u); });
             const T w = sc.W[0][i] * WYq;
             const bool anyph = HASPH && ((i == P && xph) || (q == P && yph) || zp);
             double pr0 = 1.0, pi0 = 0.0, pr1 = 1.0, pi1 = 0.0;          // conj phase of planes < P / of the wrapped top plane
@@ -587,7 +594,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
                         const int koc = live ? ko : 0;
                         const long long zq = nt == 0 ? (e == 0 ? zq0 : zq1) : (e == 0 ? zq8 : zq9);
 #pragma unroll
-                        for (int mt = 0; mt < 2; ++mt) {
+                        for (int mt = 0; mt < MTW; ++mt) {
                             Val val;
                             val.a = w * acc[mt].d[nt][0][e];
                             val.b = NR == 2 ? w * acc[mt].d[nt][NR - 1][e] : (T)0;
