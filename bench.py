@@ -113,6 +113,18 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def aggregate_over_ranks(ms_local, units_per_rank, world, dist=None, device="cpu"):
+    """N > 1: every rank filtered its own block of `units_per_rank` units in `ms_local` ms; no data-path collective -- the
+    only cross-rank step is this MAX of the device-timed durations.  Returns (max ms over ranks, whole-job units per second)."""
+    ms = float(ms_local)
+    if dist is not None and world > 1:
+        import torch
+        t = torch.tensor([ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms, world * units_per_rank / (ms * 1e-3)
+
+
 def units_per_step(cfg, nvec):
     return 2.0 * cfg.nnodes * nvec * cfg.degree
 
@@ -555,10 +567,7 @@ def run_ours(args, cfg):
     launches = B.chfsi_last_launch_count() * args.steps
     clocks = sampler.stop() if rank == 0 else None
     dev = f"cuda:{local}"
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total, _ = aggregate_over_ranks(ms_total, 0.0, world, dist, dev)
     ms_step = ms_total / args.steps
     value = world * units_per_step(cfg, nvec) / (ms_step * 1e-3)
     assert bool(torch.isfinite(torch.view_as_real(w.Y[:, :, :8])).all()), "filter output is not finite"
