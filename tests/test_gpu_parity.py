@@ -443,3 +443,48 @@ def test_filter_fp32_stored_multivectors(env, p, ncell, kfrac, nvec, degree, chu
             pb.gpu_filter(X, None, degree, a, b, a0, B.FP32_STORED, B.RECUR_STANDARD)
     finally:
         pb.close()
+
+
+def test_ragged_chunk_at_the_end_of_an_exact_size_allocation(env):
+    """the TMA boxes of a ragged last chunk (nvec = ld = 11, chunks of 4) must not read past the caller's allocation.
+    Run in a subprocess with the caching allocator switched off (every tensor is its own cudaMalloc) and with X and Y placed
+    at the very end of allocations that are whole 2 MiB pages: an out-of-bounds TMA read lands outside the mapping."""
+    import os
+    import subprocess
+    import sys
+    import textwrap
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = textwrap.dedent("""
+        import sys, numpy as np, torch
+        sys.path.insert(0, %r)
+        from paper_2605_30128_b200 import binding as B, inputs as inp
+        cfg = inp.tiny_config(ncell=3, p=4, L=6.0, kfrac=(0.25, 0.0, 0.0), nvec=11, natoms=2, nproj=8, ngauss=3)
+        mesh = B.chfsi_mesh_create(cfg.ncell, cfg.L, cfg.p, cfg.kfrac, 0)
+        hi = inp.make_hamiltonian(cfg, B.chfsi_mesh_node_coords(mesh))
+        B.chfsi_ham_set(mesh, hi.V, hi.Bx, hi.By, hi.Bz, hi.supp_off, hi.supp_node, hi.nproj, hi.P, hi.D)
+        X = inp.make_vectors(cfg.nnodes, 11)
+        need = X.nbytes
+        page = 2 << 20
+        def at_end(fill):
+            raw = torch.empty(((need + page - 1) // page) * page, dtype=torch.uint8, device="cuda")
+            t = raw[raw.numel() - need:].view(torch.complex128).view(cfg.nnodes, 2, 11)
+            t.copy_(torch.from_numpy(fill))
+            return raw, t
+        rawx, Xd = at_end(X)
+        rawy, Yd = at_end(np.zeros_like(X))
+        lam = np.zeros(11)
+        out = {}
+        for prec in (B.FP64, B.FP32, B.FP32_STORED, B.TF32):
+            for chunk in (4, 0):
+                work = torch.empty(B.chfsi_workspace_bytes(mesh, prec, B.RECUR_RESIDUAL, chunk or 11), dtype=torch.uint8, device="cuda")
+                B.chfsi_cheb_filter(mesh, prec, B.RECUR_RESIDUAL, 6, 1.0, 60.0, -3.0, Xd, lam, Yd, work, chunk=chunk)
+                torch.cuda.synchronize()
+                out[(prec, chunk)] = Yd.cpu().numpy().copy()
+            a, b = out[(prec, 4)], out[(prec, 0)]
+            tol = 1e-12 if prec == B.FP64 else (1e-5 if prec != B.TF32 else 5e-3)
+            assert np.isfinite(a).all() and np.linalg.norm(a - b) <= tol * np.linalg.norm(b), prec
+        print("OK")
+    """ % root)
+    envv = dict(os.environ, PYTORCH_NO_CUDA_MEMORY_CACHING="1")
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, env=envv, timeout=600)
+    assert r.returncode == 0 and "OK" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
