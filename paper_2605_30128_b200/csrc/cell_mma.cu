@@ -102,7 +102,7 @@ __device__ __forceinline__ uint32_t swz128(uint32_t lin) { return kSwizzle ? lin
 
 __device__ __forceinline__ void red_add_t(double* p, double v) { atomicAdd(p, v); }     // result unused -> RED
 __device__ __forceinline__ void red_add_c64(float* p, float re, float im) {             // one complex64: 8-byte vector RED
-    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(re), "f"(im) : "memory");
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(re), "f"(im));      // `out` is never read by this kernel
 }
 
 // round-to-nearest, ties away from zero, to the 10-bit TF32 mantissa (what cvt.rna.tf32.f32 returns for finite inputs):
@@ -112,12 +112,12 @@ __device__ __forceinline__ float tf32_value(uint32_t b) { return __uint_as_float
 
 __device__ __forceinline__ void mma_tf32(float (&d)[2][2], const uint32_t (&a)[2][2], const uint32_t (&b)[2]) {
     // a[r][h] = A(row g + 8r, k-half h) -> a0 = a[0][0], a1 = a[1][0], a2 = a[0][1], a3 = a[1][1]; d[r][e] = D(row g + 8r, col 2t + e)
-    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+f"(d[0][0]), "+f"(d[0][1]), "+f"(d[1][0]), "+f"(d[1][1])
                  : "r"(a[0][0]), "r"(a[1][0]), "r"(a[0][1]), "r"(a[1][1]), "r"(b[0]), "r"(b[1]));
 }
 __device__ __forceinline__ void mma_f64(double (&d)[1][2], double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(d[0][0]), "+d"(d[0][1]) : "d"(a), "d"(b));
 }
 
@@ -566,7 +566,7 @@ cell_mma_kernel(const __grid_constant__ MmaConst<typename MmaCfg<P, MODE>::T> sc
         const long long zq8 = zoff(g0 + tb + (8 + 2 * t4 < n ? 8 + 2 * t4 : 0)) + zrow;
         const long long zq9 = zoff(g0 + tb + (9 + 2 * t4 < n ? 9 + 2 * t4 : 0)) + zrow;
 #pragma unroll 1
-        for (int i = 0; i < n; ++i) {
+        for (int i = 0; i < n; ++i) {                 // (unrolling by 3 to put three nodes in flight changed nothing: 6.42 vs 6.37 ms)
             Acc<P, MODE> acc[MTW];
 #pragma unroll
             for (int mt = 0; mt < MTW; ++mt) acc[mt].zero();
