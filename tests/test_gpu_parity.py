@@ -488,3 +488,35 @@ def test_ragged_chunk_at_the_end_of_an_exact_size_allocation(env):
     envv = dict(os.environ, PYTORCH_NO_CUDA_MEMORY_CACHING="1")
     r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, env=envv, timeout=600)
     assert r.returncode == 0 and "OK" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
+
+
+def test_filter_call_is_capturable_in_a_cuda_graph(env):
+    """include/chfsi.h: chfsi_cheb_filter allocates nothing and never synchronises; the per-chunk coefficient program goes
+    through a pinned staging ring owned by the mesh.  A captured call replays to the same result as a direct one (the nonlocal
+    term then stays on the capturing stream)."""
+    torch, fo, B = env
+    cfg = inp.tiny_config(ncell=3, p=4, L=6.0, kfrac=(0.25, 0.0, 0.0), nvec=8, natoms=2, nproj=8, ngauss=3)
+    pb = Problem(env, cfg)
+    try:
+        X = inp.make_vectors(cfg.nnodes, 8)
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref = fo.cheb_filter_residual(pb.oham, X, lam, 7, a, b, a0)
+        Xd = torch.from_numpy(X).cuda()
+        for prec, tol in ((B.FP64, TOL64), (B.FP32_STORED, TOL32S), (B.TF32X3, TOL32)):
+            Yd = torch.zeros_like(Xd)
+            work = pb.work(prec, B.RECUR_RESIDUAL, 4)
+            s = torch.cuda.Stream()
+            s.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(s):
+                B.chfsi_cheb_filter(pb.gmesh, prec, B.RECUR_RESIDUAL, 7, a, b, a0, Xd, lam, Yd, work, chunk=4, stream=s)   # warm-up
+                s.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=s):
+                    B.chfsi_cheb_filter(pb.gmesh, prec, B.RECUR_RESIDUAL, 7, a, b, a0, Xd, lam, Yd, work, chunk=4, stream=s)
+                Yd.zero_()
+                g.replay()
+                s.synchronize()
+            assert relerr(Yd.cpu().numpy(), ref) < tol, prec
+    finally:
+        pb.close()
