@@ -14,7 +14,7 @@ namespace chfsi {
 //      (i = ty + 16 a, j = tx + 16 b); K-slabs of 8 rows, double buffered through registers.
 constexpr int PT = 64, PK = 8;
 
-__global__ void __launch_bounds__(256) rr_project_kernel(const double2* __restrict__ A, long long lda, const double2* __restrict__ B,
+__global__ void __launch_bounds__(256, 2) rr_project_kernel(const double2* __restrict__ A, long long lda, const double2* __restrict__ B,
                                                          long long ldb, long long nrows, int nvec, long long rows_per_cta,
                                                          const double* __restrict__ mass, int hermitian, double2* __restrict__ S) {
     const int ti = blockIdx.y, tj = blockIdx.x;
@@ -103,7 +103,7 @@ __global__ void rr_split_q_kernel(const double2* __restrict__ Q, int nvec, doubl
 // C[r][j] = Y[r][j] dq[j] (FP64) + sum_i (TC)Y[r][i] Qo[i][j] (arithmetic and accumulation in TC).  Tile RT rows x 64 columns,
 // 16 x 16 threads, RA x 4 outputs per thread (r = ty + 16 a, j = tx + 16 b); K-slabs of 8 columns of Y.
 template <typename TC, typename TC2, int RA>
-__global__ void __launch_bounds__(256) rr_rotate_kernel(const double2* __restrict__ Y, long long ldy, const TC2* __restrict__ Qo,
+__global__ void __launch_bounds__(256, 2) rr_rotate_kernel(const double2* __restrict__ Y, long long ldy, const TC2* __restrict__ Qo,
                                                         const double2* __restrict__ dq, long long nrows, int nvec,
                                                         double2* __restrict__ C, long long ldc) {
     constexpr int RT = 16 * RA, KT = 8;
@@ -209,7 +209,8 @@ chfsi_status chfsi_rr_project(const chfsi_mesh* mesh, long long nrows, int nvec,
     const int nt = (nvec + PT - 1) / PT;
     const long long tiles = hermitian ? (long long)nt * (nt + 1) / 2 : (long long)nt * nt;
     // split the rows so that the live tiles fill the GPU a few times over; slabs are multiples of PK rows
-    long long nz = (4 * 148 + tiles - 1) / tiles;
+    long long nz = (8 * 148) / tiles;                      // live CTAs = a whole number of waves of 2 CTAs per SM (rounded down)
+    if (nz < 1) nz = 1;
     if (nz > 65535) nz = 65535;
     long long rows_per = ((nrows + nz - 1) / nz + PK - 1) / PK * PK;
     if (rows_per < PK) rows_per = PK;
