@@ -480,6 +480,11 @@ def extra_kernels(torch, B, device, hbm_peak, pipe):
         rows.append({"kernel": "poisson Kx (memset + cell kernel)", "nodes": cfg.nnodes, "real_columns": 4 * nv, "ms": round(t, 4),
                      "dof_per_s": float(f"{dofs / (t * 1e-3):.4g}"), "bound": "hbm", "achieved_GBs": round(nbytes / (t * 1e-3) / 1e9, 1),
                      "peak_GBs": hbm_peak, "frac": round(nbytes / (t * 1e-3) / 1e9 / hbm_peak, 4), "dtype": "f64"})
+        B.chfsi_poisson_set_quadrature(mesh, 1)
+        t = timed(lambda: B.chfsi_poisson_apply_K(mesh, U, W), reps=3)
+        B.chfsi_poisson_set_quadrature(mesh, 0)
+        rows.append({"kernel": "poisson Kx, Gauss-Legendre form (the paper's six-contraction pipeline; untuned)", "nodes": cfg.nnodes,
+                     "real_columns": 4 * nv, "ms": round(t, 4), "dof_per_s": float(f"{dofs / (t * 1e-3):.4g}"), "dtype": "f64"})
         mass = torch.from_numpy(B.chfsi_mesh_mass(mesh)).to(dev)
         F = U * mass[:, None, None]
         Fr = torch.view_as_real(F)

@@ -231,6 +231,11 @@ chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const v
  *   runs maxit iterations without synchronising).  iters_host / resnorm_host (host, 4 nvec each, may be NULL; reading them
  *   synchronises): iterations taken and final residual norm per column.  work: chfsi_poisson_workspace_bytes, 256-byte aligned.
  *   FP64 throughout. */
+/* chfsi_poisson_set_quadrature: rule 0 (default) = GLL collocation as above; rule 1 = the paper's Kx with p + 1 Gauss-Legendre points
+ *   per direction ("six batched tensor contractions covering interpolation of nodal values to quadrature points, application of the
+ *   per-cell Jacobian, and integration back"): a different, consistent-mass discretisation of the same operator; every
+ *   chfsi_poisson_* call then uses it (its own Kx kernel, its own diag(K)).  Setup call (may allocate).  Needs >= 2 cells per direction. */
+chfsi_status chfsi_poisson_set_quadrature(chfsi_mesh* mesh, int rule);
 chfsi_status chfsi_poisson_kdiag(const chfsi_mesh* mesh, double* kdiag_host);
 chfsi_status chfsi_poisson_apply_K(const chfsi_mesh* mesh, int nvec, const void* U, long long ldu, void* W, long long ldw,
                                    void* cuda_stream);

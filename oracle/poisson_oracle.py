@@ -136,7 +136,7 @@ def k_diag(mesh, rule: str = "gll") -> np.ndarray:
     return d
 
 
-def lanczos_bounds_scaled(mesh, kd: np.ndarray, start: np.ndarray, steps: int = 10):
+def lanczos_bounds_scaled(mesh, kd: np.ndarray, start: np.ndarray, steps: int = 10, rule: str = "gll"):
     """Largest Ritz value (plus the residual norm) of K_diag^-1 K from a `steps`-step Lanczos run in the K_diag inner
     product; returns (lmin, lmax) with lmin = lmax / 30 (reading P4)."""
     v = start - np.sum(kd * start) / np.sum(kd)
@@ -144,7 +144,7 @@ def lanczos_bounds_scaled(mesh, kd: np.ndarray, start: np.ndarray, steps: int = 
     vprev = np.zeros_like(v)
     alphas, betas, beta = [], [], 0.0
     for j in range(steps):
-        f = apply_K(mesh, v[:, None])[:, 0] / kd - beta * vprev
+        f = apply_K(mesh, v[:, None], rule)[:, 0] / kd - beta * vprev
         alpha = float(np.sum(kd * v * f))
         f = f - alpha * v
         alphas.append(alpha)
@@ -157,7 +157,7 @@ def lanczos_bounds_scaled(mesh, kd: np.ndarray, start: np.ndarray, steps: int = 
     return lmax / 30.0, lmax
 
 
-def cheb_jacobi(mesh, kd: np.ndarray, r: np.ndarray, m: int, lmin: float, lmax: float) -> np.ndarray:
+def cheb_jacobi(mesh, kd: np.ndarray, r: np.ndarray, m: int, lmin: float, lmax: float, rule: str = "gll") -> np.ndarray:
     """z = chi(K_diag^-1 K) K_diag^-1 r with the degree-m Chebyshev approximation of 1/lambda on [lmin, lmax]: the
     three-term Chebyshev iteration for K z = r from z = 0 (reading P4); m - 1 applications of K."""
     theta, delta = 0.5 * (lmax + lmin), 0.5 * (lmax - lmin)
@@ -167,22 +167,22 @@ def cheb_jacobi(mesh, kd: np.ndarray, r: np.ndarray, m: int, lmin: float, lmax: 
     z = d.copy()
     for _ in range(1, m):
         rho_new = 1.0 / (2.0 * sigma - rho)
-        res = r - apply_K(mesh, z)
+        res = r - apply_K(mesh, z, rule)
         d = rho_new * rho * d + (2.0 * rho_new / delta) * (res / kd[:, None])
         z = z + d
         rho = rho_new
     return z
 
 
-def pcg(mesh, f: np.ndarray, m: int, lmin: float, lmax: float, tol: float, maxit: int):
+def pcg(mesh, f: np.ndarray, m: int, lmin: float, lmax: float, tol: float, maxit: int, rule: str = "gll"):
     """Algorithm 2 for every column of f [M, ncols] independently (reading P5).  Returns (x, iterations per
     column, final residual norms).  Notation of the paper: r = K x - f, delta = r . z, eta = p . w, gamma = |r|^2."""
     f = np.asarray(f, dtype=np.float64)
-    kd = k_diag(mesh)
+    kd = k_diag(mesh, rule)
     nc = f.shape[1]
     x = np.zeros_like(f)
     r = -f.copy()                                      # r = K x - f with x = 0
-    z = cheb_jacobi(mesh, kd, r, m, lmin, lmax)
+    z = cheb_jacobi(mesh, kd, r, m, lmin, lmax, rule)
     p = -z
     delta = np.sum(r * z, axis=0)
     gamma = np.sum(r * r, axis=0)
@@ -191,12 +191,12 @@ def pcg(mesh, f: np.ndarray, m: int, lmin: float, lmax: float, tol: float, maxit
     for _ in range(maxit):
         if not active.any():
             break
-        w = apply_K(mesh, p)                                           # 1: Kx kernel
+        w = apply_K(mesh, p, rule)                                     # 1: Kx kernel
         eta = np.sum(p * w, axis=0)                                    # 2: dot kernel
         alpha = np.where(active, delta / np.where(eta != 0, eta, 1.0), 0.0)   # 3
         x += alpha * p                                                 # 4: fused update
         r += alpha * w
-        z = cheb_jacobi(mesh, kd, r, m, lmin, lmax)                    # 5: Chebyshev preconditioner
+        z = cheb_jacobi(mesh, kd, r, m, lmin, lmax, rule)              # 5: Chebyshev preconditioner
         delta_new = np.sum(r * z, axis=0)                              # 6: fused dot
         gamma = np.where(active, np.sum(r * r, axis=0), gamma)
         beta = np.where(active, delta_new / np.where(delta != 0, delta, 1.0), 0.0)   # 8

@@ -27,7 +27,7 @@ EXPORTS = [
     "chfsi_bfp_stream_bytes", "chfsi_bfp_encode", "chfsi_bfp_decode", "chfsi_bfp_gather_encode",
     "chfsi_bfp_decode_scatter_add",
     "chfsi_rr_project", "chfsi_rr_rotate_workspace_bytes", "chfsi_rr_rotate", "chfsi_measure_pipe_peaks",
-    "chfsi_poisson_kdiag", "chfsi_poisson_apply_K", "chfsi_poisson_workspace_bytes", "chfsi_poisson_pcg",
+    "chfsi_poisson_set_quadrature", "chfsi_poisson_kdiag", "chfsi_poisson_apply_K", "chfsi_poisson_workspace_bytes", "chfsi_poisson_pcg",
     "chfsi_last_launch_count", "chfsi_last_error", "chfsi_version",
 ]
 
@@ -73,6 +73,7 @@ def lib() -> C.CDLL:
     L.chfsi_rr_rotate_workspace_bytes.argtypes = [C.c_int, C.POINTER(C.c_size_t)]
     L.chfsi_rr_rotate.argtypes = [C.c_int, C.c_longlong, C.c_int, vp, C.c_longlong, vp, vp, C.c_longlong, vp, C.c_size_t, vp]
     L.chfsi_measure_pipe_peaks.argtypes = [C.c_int, dp]
+    L.chfsi_poisson_set_quadrature.argtypes = [vp, C.c_int]
     L.chfsi_poisson_kdiag.argtypes = [vp, dp]
     L.chfsi_poisson_apply_K.argtypes = [vp, C.c_int, vp, C.c_longlong, vp, C.c_longlong, vp]
     L.chfsi_poisson_workspace_bytes.argtypes = [vp, C.c_int, C.POINTER(C.c_size_t)]
@@ -275,6 +276,11 @@ def chfsi_measure_pipe_peaks(device=0) -> dict:
 
 
 # ---- Poisson solve ----------------------------------------------------------------
+def chfsi_poisson_set_quadrature(mesh, rule):
+    """rule 0: GLL collocation (default); 1: Gauss-Legendre, the paper's Kx."""
+    _check(lib().chfsi_poisson_set_quadrature(mesh, int(rule)))
+
+
 def chfsi_poisson_kdiag(mesh) -> np.ndarray:
     kd = np.empty(chfsi_mesh_num_nodes(mesh), dtype=np.float64)
     _check(lib().chfsi_poisson_kdiag(mesh, _dptr(kd)))

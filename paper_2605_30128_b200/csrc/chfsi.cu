@@ -243,7 +243,7 @@ chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
         if (m->side) cudaStreamDestroy(m->side);
         for (cudaEvent_t e : m->stage_ev) if (e) cudaEventDestroy(e);
         if (m->h_stage) cudaFreeHost(m->h_stage);
-        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF); cudaFree(m->dMass); cudaFree(m->dKdiag);
+        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF); cudaFree(m->dMass); cudaFree(m->dKdiag); cudaFree(m->dKdiagGL); delete m->gl;
         free_nonlocal(m->nl);
     }
     delete m;

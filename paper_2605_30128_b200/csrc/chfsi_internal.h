@@ -60,6 +60,15 @@ struct CellArgs {
     int store_f32;
 };
 
+// tables of the Gauss-Legendre form of the Poisson operator (poisson_gl.cu)
+struct GlTables {
+    double Bm[kMaxN][kMaxN];    // B[q][i]  = l_i(xq_q): nodal values -> Gauss points
+    double Dq[kMaxN][kMaxN];    // Dq[q][r] = collocation derivative at the Gauss points (G B^-1)
+    double wq[kMaxN];           // Gauss weights
+    double coef[3];             // J (2/h_d)^2
+    int nc[3], n1[3];
+};
+
 struct ProjItem { int atom; int start; int count; };   // a slice of an atom's support list
 
 struct NonlocalDev {
@@ -124,6 +133,9 @@ struct chfsi_mesh {
     double* dF = nullptr;               // packed fields [M][4] = V+Bz, V-Bz, Bx, By (march kernel)
     double* dMass = nullptr;            // node masses m_I [M] (Rayleigh-Ritz projection, Poisson solver); built in chfsi_ham_set
     double* dKdiag = nullptr;           // diag(K) of the stiffness matrix K = 2 x kinetic part [M] (Poisson preconditioner); built in chfsi_ham_set
+    double* dKdiagGL = nullptr;         // the same for the Gauss-Legendre form (chfsi_poisson_set_quadrature)
+    int poisson_rule = 0;               // 0: GLL collocation (the filter's Laplacian, cell kernel); 1: Gauss-Legendre (the paper's Kx)
+    chfsi::GlTables* gl = nullptr;      // host copy of the Gauss-Legendre tables
     bool bare_laplacian = false;        // the Hamiltonian set last has no local fields and no projectors (Poisson handle)
     chfsi::NonlocalDev nl;
     // profiling aid (chfsi_profile_enable / chfsi_profile_read)
@@ -175,6 +187,10 @@ cudaError_t launch_cell_xyz(const chfsi_mesh* m, chfsi_prec prec, const CellArgs
 // tensor-core cell kernel (cell_mma.cu): mma.sync TF32 / 3xTF32 on complex64 storage, mma.sync FP64 on complex128 storage
 bool mma_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
 cudaError_t launch_cell_mma(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
+// Gauss-Legendre form of the Poisson operator (poisson_gl.cu)
+bool build_gl_tables(const chfsi_mesh* m, GlTables& tb, std::vector<double>* k1_out, std::vector<double>* m1_out);
+cudaError_t launch_kx_gl(const chfsi_mesh* m, const GlTables& tb, int nvec, const double* U, long long ldu, double* W, long long ldw,
+                         double cH, cudaStream_t st);
 void set_error(const std::string& s);
 void count_launch(int n = 1);
 }  // namespace chfsi

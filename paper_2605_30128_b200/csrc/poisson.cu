@@ -11,6 +11,7 @@
 // (PAPER.md:195).  All FP64.
 #include <cmath>
 #include <cstdint>
+#include <new>
 #include <vector>
 
 #include "chfsi_internal.h"
@@ -146,7 +147,7 @@ static size_t al256(size_t b) { return (b + 255) / 256 * 256; }
 
 static chfsi_status poisson_check(const chfsi_mesh* m, int nvec, const char* who) {
     if (!m) return pfail(CHFSI_EINVAL, "poisson: mesh is NULL");
-    if (!m->ham_set || !m->bare_laplacian || !m->dKdiag)
+    if (!m->ham_set || !m->bare_laplacian || !m->dKdiag || (m->poisson_rule == 1 && (!m->gl || !m->dKdiagGL)))
         return pfail(CHFSI_ESTATE, "poisson: the handle's Hamiltonian must be the bare Laplacian (chfsi_ham_set with NULL fields and no atoms)");
     if (m->mc.has_phase) return pfail(CHFSI_EINVAL, "poisson: real periodic fields only (kfrac must be 0)");
     if (nvec < 1) return pfail(CHFSI_EINVAL, "poisson: nvec must be >= 1");
@@ -157,6 +158,16 @@ static chfsi_status poisson_check(const chfsi_mesh* m, int nvec, const char* who
 // W (+)= cH * 2 * (kinetic part)(U) + cR R through the library's cell kernel
 static chfsi_status kx_launch(const chfsi_mesh* m, int nvec, const double* U, long long ldu, double* W, long long ldw, double cH,
                               const double* R, long long ldr, const double* ones, cudaStream_t st) {
+    if (m->poisson_rule == 1) {
+        // the paper's Gauss-Legendre Kx (poisson_gl.cu): W (zeroed by the caller) = R + cH K U
+        if (R) {
+            PCU(cudaMemcpy2DAsync(W, (size_t)ldw * 16, R, (size_t)ldr * 16, (size_t)nvec * 16, (size_t)2 * m->nnodes, cudaMemcpyDeviceToDevice, st));
+            count_launch();
+        }
+        const cudaError_t e = launch_kx_gl(m, *m->gl, nvec, U, ldu, W, ldw, cH, st);
+        if (e != cudaSuccess) { set_error(std::string("poisson Kx (Gauss-Legendre): ") + cudaGetErrorString(e)); return CHFSI_ECUDA; }
+        return CHFSI_OK;
+    }
     CellArgs ca{};
     ca.in = U; ca.ld_in = ldu; ca.out = W; ca.ld_out = ldw;
     ca.R = R; ca.ld_R = ldr; ca.cin = nullptr; ca.cR = R ? ones : nullptr;
@@ -171,7 +182,49 @@ extern "C" {
 chfsi_status chfsi_poisson_kdiag(const chfsi_mesh* m, double* kdiag_host) {
     if (!m || !kdiag_host) return pfail(CHFSI_EINVAL, "poisson_kdiag: NULL argument");
     if (!m->dKdiag) return pfail(CHFSI_ESTATE, "poisson_kdiag: chfsi_ham_set has not been called");
-    PCU(cudaMemcpy(kdiag_host, m->dKdiag, (size_t)m->nnodes * sizeof(double), cudaMemcpyDeviceToHost));
+    const double* src = m->poisson_rule == 1 ? m->dKdiagGL : m->dKdiag;
+    if (!src) return pfail(CHFSI_ESTATE, "poisson_kdiag: no diagonal for the selected quadrature");
+    PCU(cudaMemcpy(kdiag_host, src, (size_t)m->nnodes * sizeof(double), cudaMemcpyDeviceToHost));
+    return CHFSI_OK;
+}
+
+chfsi_status chfsi_poisson_set_quadrature(chfsi_mesh* m, int rule) {
+    if (!m) return pfail(CHFSI_EINVAL, "poisson_set_quadrature: mesh is NULL");
+    if (rule != 0 && rule != 1) return pfail(CHFSI_EINVAL, "poisson_set_quadrature: rule must be 0 (GLL) or 1 (Gauss-Legendre)");
+    if (rule == 1 && !m->gl) {
+        if (m->nc[0] < 2 || m->nc[1] < 2 || m->nc[2] < 2) return pfail(CHFSI_EINVAL, "poisson_set_quadrature: needs at least two cells per direction");
+        GlTables* tb = new (std::nothrow) GlTables;
+        if (!tb) return pfail(CHFSI_ENOMEM, "poisson_set_quadrature: out of host memory");
+        std::vector<double> k1, m1;
+        if (!build_gl_tables(m, *tb, &k1, &m1)) { delete tb; return pfail(CHFSI_ECUDA, "poisson_set_quadrature: table construction failed"); }
+        // diag(K): K_e = sum_d coef_d K1 (x) M1 (x) M1 is separable, so the assembled diagonal is a sum of products of assembled 1-D diagonals
+        const int p = m->p;
+        std::vector<double> ka[3], ma[3];
+        for (int d = 0; d < 3; ++d) {
+            const int n1 = m->mc.n1[d];
+            ka[d].assign(n1, 0.0); ma[d].assign(n1, 0.0);
+            for (int g = 0; g < n1; ++g) {
+                const int a = g % p;
+                ka[d][g] = k1[a] + (a == 0 ? k1[p] : 0.0);
+                ma[d][g] = m1[a] + (a == 0 ? m1[p] : 0.0);
+            }
+        }
+        std::vector<double> kd((size_t)m->nnodes);
+        const int nx = m->mc.n1[0], ny = m->mc.n1[1], nz = m->mc.n1[2];
+        for (int iz = 0; iz < nz; ++iz)
+            for (int iy = 0; iy < ny; ++iy)
+                for (int ix = 0; ix < nx; ++ix)
+                    kd[((size_t)iz * ny + iy) * nx + ix] = tb->coef[0] * ka[0][ix] * ma[1][iy] * ma[2][iz] + tb->coef[1] * ma[0][ix] * ka[1][iy] * ma[2][iz] +
+                                                          tb->coef[2] * ma[0][ix] * ma[1][iy] * ka[2][iz];
+        int prev = 0;
+        cudaGetDevice(&prev); cudaSetDevice(m->device);
+        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&m->dKdiagGL), kd.size() * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemcpy(m->dKdiagGL, kd.data(), kd.size() * sizeof(double), cudaMemcpyHostToDevice);
+        cudaSetDevice(prev);
+        if (e != cudaSuccess) { delete tb; set_error(std::string("poisson_set_quadrature: ") + cudaGetErrorString(e)); return CHFSI_ECUDA; }
+        m->gl = tb;
+    }
+    m->poisson_rule = rule;
     return CHFSI_OK;
 }
 
@@ -238,10 +291,11 @@ chfsi_status chfsi_poisson_pcg(const chfsi_mesh* m, int nvec, const void* F, lon
     const unsigned gdot = (unsigned)((M + npb - 1) / npb);
     const int tdot = ncol < 512 ? ((ncol + 31) / 32) * 32 : 512;
     const double theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
+    const double* kdiag = m->poisson_rule == 1 ? m->dKdiagGL : m->dKdiag;
 
     // z = P^-1 r: Chebyshev-Jacobi, cheb_degree - 1 applications of K
     auto precondition = [&]() -> chfsi_status {
-        pois_pass_kernel<PP_CHEB0><<<gpass, 256, 0, st>>>(d, z, r, nullptr, nvec, nvec, nvec, M, m->dKdiag, nullptr, nullptr, theta, 0.0);
+        pois_pass_kernel<PP_CHEB0><<<gpass, 256, 0, st>>>(d, z, r, nullptr, nvec, nvec, nvec, M, kdiag, nullptr, nullptr, theta, 0.0);
         count_launch();
         double rho = 1.0 / sigma;
         for (int k = 1; k < cheb_degree; ++k) {
@@ -249,7 +303,7 @@ chfsi_status chfsi_poisson_pcg(const chfsi_mesh* m, int nvec, const void* F, lon
             PCU(cudaMemsetAsync(w, 0, (size_t)2 * M * nvec * 16, st)); count_launch();
             chfsi_status s2 = kx_launch(m, nvec, z, nvec, w, nvec, -1.0, r, nvec, ones, st);      // t = r - K z in one pass
             if (s2 != CHFSI_OK) return s2;
-            pois_pass_kernel<PP_CHEB><<<gpass, 256, 0, st>>>(d, z, w, nullptr, nvec, nvec, nvec, M, m->dKdiag, nullptr, nullptr,
+            pois_pass_kernel<PP_CHEB><<<gpass, 256, 0, st>>>(d, z, w, nullptr, nvec, nvec, nvec, M, kdiag, nullptr, nullptr,
                                                               rho_new * rho, 2.0 * rho_new / delta);
             count_launch();
             rho = rho_new;

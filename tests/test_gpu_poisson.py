@@ -108,6 +108,46 @@ def test_pcg_matches_the_oracle(env, po, p, ncell, L, nvec, m):
         B.chfsi_mesh_destroy(mesh)
 
 
+@pytest.mark.parametrize("p,ncell,L,nvec", [(2, (3, 2, 2), (3.0, 2.0, 2.5), 3), (3, (2, 2, 2), (4.0, 4.0, 4.0), 2), (6, (2, 2, 2), (4.0, 5.0, 4.0), 5),
+                                            (8, (2, 2, 2), (4.0, 4.0, 6.0), 4)])
+def test_gauss_legendre_kx_and_pcg_match_the_oracle(env, po, p, ncell, L, nvec):
+    """chfsi_poisson_set_quadrature(mesh, 1): the paper's Kx (interpolation to p + 1 Gauss points, Jacobian, integration back)
+    against the oracle's rule = "gl" pipeline, its diag(K), and Algorithm 2 on top of it; then back to the default rule."""
+    torch, fo, B = env
+    omesh = fo.Mesh(ncell, L, p)
+    mesh = _handle(B, ncell, L, p)
+    try:
+        B.chfsi_poisson_set_quadrature(mesh, 1)
+        rng = np.random.default_rng(20 + p)
+        u = rng.standard_normal((omesh.nnodes, 4 * nvec))
+        ref = po.apply_K(omesh, u, "gl")
+        Ud = torch.from_numpy(_block(u, omesh.nnodes, nvec)).cuda()
+        Wd = torch.full_like(Ud, float("nan"))
+        B.chfsi_poisson_apply_K(mesh, Ud, Wd)
+        got = _cols(Wd.cpu().numpy())
+        assert relerr(got, ref) < 1e-13 and np.abs(got - ref).max() < 1e-12 * np.abs(ref).max()
+        kd = B.chfsi_poisson_kdiag(mesh)
+        kdo = po.k_diag(omesh, "gl")
+        assert np.abs(kd - kdo).max() < 1e-13 * kdo.max()
+        if p <= 6:
+            f = rng.standard_normal((omesh.nnodes, 4 * nvec)) * omesh.mass[:, None]
+            f -= f.mean(axis=0)
+            lmin, lmax = po.lanczos_bounds_scaled(omesh, kd, rng.standard_normal(omesh.nnodes), rule="gl")
+            xo, ito, _ = po.pcg(omesh, f, 3, lmin, lmax, 1e-10, 400, rule="gl")
+            Fd = torch.from_numpy(_block(f, omesh.nnodes, nvec)).cuda()
+            Xd = torch.full_like(Fd, float("nan"))
+            work = torch.empty(B.chfsi_poisson_workspace_bytes(mesh, nvec), dtype=torch.uint8, device="cuda")
+            it, res = B.chfsi_poisson_pcg(mesh, Fd, Xd, 3, lmin, lmax, 1e-10, 400, work)
+            x = _cols(Xd.cpu().numpy())
+            assert (res < 1e-10).all() and np.abs(it.reshape(-1) - ito).max() <= 1
+            assert np.abs(x - xo).max() < 1e-8 * np.abs(xo).max()
+        B.chfsi_poisson_set_quadrature(mesh, 0)
+        B.chfsi_poisson_apply_K(mesh, Ud, Wd)
+        assert relerr(_cols(Wd.cpu().numpy()), po.apply_K(omesh, u)) < 1e-13
+    finally:
+        B.chfsi_mesh_destroy(mesh)
+
+
 def test_cosine_charges_at_config1_size_and_error_codes(env, po):
     """configs[1]'s mesh (8^3 cells, p = 6, 110,592 nodes), 16 right-hand sides = 16 different plane-wave charges
     rho = cos(k . r): V = 4 pi rho / |k|^2 analytically; bounds from the harness-side Lanczos run."""

@@ -111,6 +111,21 @@ def test_pcg_reaches_the_pseudo_inverse_solution_and_preconditioning_cuts_iterat
     assert its[5] < its[3] < its[1]
 
 
+def test_pcg_with_the_gauss_rule_reaches_its_pseudo_inverse_solution():
+    """The paper's Gauss-Legendre form through the same Algorithm 2 (rule = "gl" is only passed through to apply_K / k_diag)."""
+    mesh = fo.Mesh((2, 2, 2), (4.0, 4.0, 5.0), 3)
+    K = _dense_K(mesh, "gl")
+    rng = np.random.default_rng(4)
+    f = rng.standard_normal((mesh.nnodes, 2)); f -= f.mean(axis=0)
+    kd = po.k_diag(mesh, "gl")
+    assert np.abs(kd - np.diag(K)).max() < 1e-12 * kd.max()
+    lmin, lmax = po.lanczos_bounds_scaled(mesh, kd, rng.standard_normal(mesh.nnodes), rule="gl")
+    x, it, res = po.pcg(mesh, f, 3, lmin, lmax, 1e-10, 500, rule="gl")
+    xref = np.linalg.lstsq(K, f, rcond=None)[0]
+    xref -= np.sum(mesh.mass[:, None] * xref, axis=0) / mesh.mass.sum()
+    assert (res < 1e-10).all() and np.abs(x - xref).max() < 1e-8 * np.abs(xref).max()
+
+
 def test_cosine_charge_is_solved_spectrally():
     """-laplace V = 4 pi rho with rho = cos(2 pi x / Lx) cos(2 pi z / Lz) has V = 4 pi rho / |k|^2; the FE solution (load
     f = 4 pi m rho, reading P3) approaches it spectrally as p rises (same mesh family as pin P9 of the filter oracle)."""
