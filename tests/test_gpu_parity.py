@@ -520,3 +520,58 @@ def test_filter_call_is_capturable_in_a_cuda_graph(env):
             assert relerr(Yd.cpu().numpy(), ref) < tol, prec
     finally:
         pb.close()
+
+
+def test_two_meshes_on_two_host_threads_and_streams_are_independent(env):
+    """include/chfsi.h: "a mesh handle is used from one host thread at a time ...; different meshes are independent".  Two host
+    threads, each with its own mesh (different degree p, so different kernel instantiations set their attributes concurrently),
+    its own stream and its own precision, filter repeatedly at the same time; every result must match the oracle as in the
+    serial tests, and the thread-local error state of one thread must not leak into the other."""
+    import threading
+    torch, fo, B = env
+    specs = [(4, 3, (0.25, 0, 0), 10, 9, B.FP64, TOL64), (6, 2, (0, 0.5, 0), 12, 11, B.FP32_STORED, TOL32S)]
+    jobs = []
+    for p, ncell, kfrac, nvec, degree, prec, tol in specs:
+        cfg = inp.tiny_config(ncell=ncell, p=p, L=2.0 * ncell, kfrac=kfrac, nvec=nvec, natoms=2, nproj=8, ngauss=3)
+        pb = Problem(env, cfg)
+        X = inp.make_vectors(cfg.nnodes, nvec)
+        a, b, a0 = pb.bounds()
+        lam = pb.rayleigh(X)
+        ref = fo.cheb_filter_residual(pb.oham, X, lam, degree, a, b, a0)
+        jobs.append(dict(pb=pb, X=X, lam=lam, degree=degree, abz=(a, b, a0), prec=prec, tol=tol, ref=ref, errs=[], exc=None))
+    start = threading.Barrier(len(jobs))
+
+    def run(job):
+        try:
+            pb = job["pb"]
+            stream = torch.cuda.Stream()
+            Xd = torch.from_numpy(job["X"]).cuda()
+            work = pb.work(job["prec"], B.RECUR_RESIDUAL, job["X"].shape[2])
+            torch.cuda.synchronize()
+            start.wait()
+            for it in range(6):
+                Yd = torch.full_like(Xd, float("nan"))
+                stream.wait_stream(torch.cuda.current_stream())
+                B.chfsi_cheb_filter(pb.gmesh, job["prec"], B.RECUR_RESIDUAL, job["degree"], *job["abz"], Xd, job["lam"], Yd,
+                                    work, stream=stream)
+                if it == 2:
+                    with pytest.raises(Exception):                           # an error in this thread only
+                        B.chfsi_cheb_filter(pb.gmesh, job["prec"], B.RECUR_RESIDUAL, 0, *job["abz"], Xd, job["lam"], Yd, work,
+                                            stream=stream)
+                stream.synchronize()
+                job["errs"].append(relerr(Yd.cpu().numpy(), job["ref"]))
+        except Exception as e:                                              # surfaced in the main thread below
+            job["exc"] = e
+
+    threads = [threading.Thread(target=run, args=(job,)) for job in jobs]
+    try:
+        for th in threads:
+            th.start()
+        for th in threads:
+            th.join(timeout=300)
+        for job in jobs:
+            assert job["exc"] is None, job["exc"]
+            assert len(job["errs"]) == 6 and max(job["errs"]) < job["tol"], job["errs"]
+    finally:
+        for job in jobs:
+            job["pb"].close()
