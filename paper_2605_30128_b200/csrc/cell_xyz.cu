@@ -87,7 +87,7 @@ struct XyzCfg {
     static constexpr int FACE_OFF = n * P * C * (int)sizeof(TI);
     static constexpr int IN_BYTES = n * n * C * (int)sizeof(TI);
     static constexpr int R_BYTES = P * P * C * 8;
-    static constexpr int F_BYTES = P * P * 32;
+    static constexpr int F_BYTES = P * P * (MODE == M_F32S ? 16 : 32);   // FP32-stored: the FP32 copy of the fields
     static constexpr int R_OFF = ((IN_BYTES + 127) / 128) * 128;
     static constexpr int F_OFF = R_OFF + R_BYTES;
     static constexpr int STAGE_BYTES = ((F_OFF + F_BYTES + 127) / 128) * 128;
@@ -341,11 +341,22 @@ struct XyzConsumer {
                 [[maybe_unused]] TO* p5 = outcol + (long long)(g0 + t) * PS;
 #pragma unroll
                 for (int l = 0; l < NJ; ++l) {
-                    constexpr int dummy = 0; (void)dummy;
                     const int j = RS::row(l);
                     if (j < P) {
                         // (B_x -+ i B_y) u_other: B_x * (other spin, same part) + sg * B_y * (other spin, other part)
                         const int o = j * P * C + nb;
+                        if constexpr (MODE == M_F32S) {
+                            // FP32-stored multivectors (only R and Lambda_k stay FP64): FP32 pointwise terms on
+                            // the FP32 copy of the fields; the R-term is formed in FP64 and rounded once
+                            const float4 f = *reinterpret_cast<const float4*>(reinterpret_cast<const float*>(Fs) + (j * P + a) * 4);
+                            const float in_f = vin[j];
+                            const float os = IN[o + ((col ^ (C / 2)) - col)], of = IN[o + ((col ^ (C / 2 + 1)) - col)];
+                            const float pot = fmaf(s_spin ? f.y : f.x, in_f, fmaf(f.z, os, ((float)sg * f.w) * of));
+                            float val = fmaf((float)cin, in_f, (float)sc.cHp * pot);
+                            if (ar.useR) val += (float)(cR * Rs[o]);
+                            s5[l] = val;
+                            continue;
+                        }
                         const double in_own = (double)vin[j];
                         const double o_same = (double)IN[o + ((col ^ (C / 2)) - col)];
                         const double o_flip = (double)IN[o + ((col ^ (C / 2 + 1)) - col)];
@@ -569,7 +580,7 @@ static cudaError_t launch_xyz_t(const chfsi_mesh* m, const CellArgs& a, cudaStre
             !make_map3(&mp.face[i], m, a.in, a.ld_in, a.nvec, BC, 2, nl[i], f32in))
             return cudaErrorInvalidValue;
     if (!make_map3(&mp.R, m, ar.useR ? a.R : a.in, ar.useR ? a.ld_R : a.ld_in, a.nvec, BC, 2 * P, P, ar.useR ? false : f32in) ||
-        !make_mapF(&mp.F, m, P))
+        !make_mapF(&mp.F, m, P, MODE == M_F32S))
         return cudaErrorInvalidValue;
     const bool ph = m->mc.has_phase != 0;
     // the mass of the in-term and of the potential term (residual form) needs the flags kMassIn alone

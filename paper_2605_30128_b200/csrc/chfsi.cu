@@ -243,7 +243,7 @@ chfsi_status chfsi_mesh_destroy(chfsi_mesh* m) {
         if (m->side) cudaStreamDestroy(m->side);
         for (cudaEvent_t e : m->stage_ev) if (e) cudaEventDestroy(e);
         if (m->h_stage) cudaFreeHost(m->h_stage);
-        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF); cudaFree(m->dMass); cudaFree(m->dKdiag); cudaFree(m->dKdiagGL); delete m->gl;
+        cudaFree(m->dV); cudaFree(m->dBx); cudaFree(m->dBy); cudaFree(m->dBz); cudaFree(m->dF); cudaFree(m->dF32); cudaFree(m->dMass); cudaFree(m->dKdiag); cudaFree(m->dKdiagGL); delete m->gl;
         free_nonlocal(m->nl);
     }
     delete m;
@@ -327,6 +327,10 @@ chfsi_status chfsi_ham_set(chfsi_mesh* m, const double* V, const double* Bx, con
         }
         if (m->dF == nullptr) CU(cudaMalloc(reinterpret_cast<void**>(&m->dF), (size_t)M * 32));
         CU(cudaMemcpy(m->dF, F.data(), (size_t)M * 32, cudaMemcpyHostToDevice));
+        std::vector<float> F32((size_t)M * 4);
+        for (size_t i = 0; i < F32.size(); ++i) F32[i] = (float)F[i];
+        if (m->dF32 == nullptr) CU(cudaMalloc(reinterpret_cast<void**>(&m->dF32), (size_t)M * 16));
+        CU(cudaMemcpy(m->dF32, F32.data(), (size_t)M * 16, cudaMemcpyHostToDevice));
     }
     // ---- nonlocal tables: built in a local object and swapped in only when every upload has succeeded, so that a failed
     // re-set never leaves the mesh with half-built tables (the mesh is marked unset meanwhile)

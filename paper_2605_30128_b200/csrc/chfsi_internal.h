@@ -131,6 +131,7 @@ struct chfsi_mesh {
     double* dBy = nullptr;
     double* dBz = nullptr;
     double* dF = nullptr;               // packed fields [M][4] = V+Bz, V-Bz, Bx, By (march kernel)
+    float* dF32 = nullptr;              // the same rounded to FP32 (FP32-stored mode: its pointwise terms are FP32)
     double* dMass = nullptr;            // node masses m_I [M] (Rayleigh-Ritz projection, Poisson solver); built in chfsi_ham_set
     double* dKdiag = nullptr;           // diag(K) of the stiffness matrix K = 2 x kinetic part [M] (Poisson preconditioner); built in chfsi_ham_set
     double* dKdiagGL = nullptr;         // the same for the Gauss-Legendre form (chfsi_poisson_set_quadrature)

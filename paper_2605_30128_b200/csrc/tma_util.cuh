@@ -106,15 +106,17 @@ static inline bool make_map3(CUtensorMap* map, const chfsi_mesh* m, const void* 
 }
 
 // 2-D view of the packed fields [M][4]: dim0 = the 4*N1x doubles of one x-line, dim1 = lines; box = 4P doubles x P lines
-static inline bool make_mapF(CUtensorMap* map, const chfsi_mesh* m, int P) {
+// (f32: the FP32 copy of the fields)
+static inline bool make_mapF(CUtensorMap* map, const chfsi_mesh* m, int P, bool f32 = false) {
     EncodeFn enc = get_encode();
     if (!enc) return false;
     const cuuint64_t n1x = (cuuint64_t)m->mc.n1[0];
     cuuint64_t gdim[2] = {4 * n1x, (cuuint64_t)m->mc.n1[1] * (cuuint64_t)m->mc.n1[2]};
-    cuuint64_t gstr[1] = {n1x * 32};
+    cuuint64_t gstr[1] = {n1x * (f32 ? 16u : 32u)};
     cuuint32_t box[2] = {(cuuint32_t)(4 * P), (cuuint32_t)P};
     cuuint32_t estr[2] = {1u, 1u};
-    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, m->dF, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    return enc(map, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, f32 ? (void*)m->dF32 : (void*)m->dF, gdim, gstr,
+               box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
