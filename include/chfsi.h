@@ -215,6 +215,20 @@ chfsi_status chfsi_rr_rotate_workspace_bytes(int nvec, size_t* bytes);
 chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q,
                              void* Yout, long long ldo, void* work, size_t work_bytes, void* cuda_stream);
 
+/* chfsi_rr_rotate_static: chfsi_rr_rotate (same operation, same arguments, layout and errors) for callers that
+ * cannot allocate device memory and have no workspace to pass: code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc.  The split-Q scratch is a static device array inside the library, 4,203,008 bytes
+ * (= chfsi_rr_rotate_workspace_bytes(CHFSI_RR_STATIC_MAX_NVEC)), resident on every GPU that loads the library until the
+ * process exits.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine): it launches the same
+ * two kernels as chfsi_rr_rotate on `cuda_stream`.  nvec > CHFSI_RR_STATIC_MAX_NVEC: CHFSI_EINVAL (use chfsi_rr_rotate).
+ * The device address of the array is resolved on the first call on each device (cudaGetSymbolAddress with that device
+ * current; make that first call outside stream capture).  ALL calls on a device share the one array, which keeps the last
+ * call's contents; every call rewrites the part it reads, so nothing needs clearing -- but two calls that overlap on the
+ * GPU (different streams without an ordering, or two host threads) RACE on it: serialise them. */
+#define CHFSI_RR_STATIC_MAX_NVEC 512
+chfsi_status chfsi_rr_rotate_static(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q,
+                                    void* Yout, long long ldo, void* cuda_stream);
+
 /* ---- matrix-free Poisson solve (eq. 5-6; Kx kernel and Algorithm 2) -----
  * Solves K x = f for the stiffness matrix K of -laplace on the handle's periodic mesh (GLL quadrature: K = 2 x the kinetic
  * part of H; reading P2), batched: a spinor-layout block [2 M rows][ld complex128] holds 4 nvec independent real

@@ -26,7 +26,7 @@ EXPORTS = [
     "chfsi_profile_enable", "chfsi_profile_read",
     "chfsi_bfp_stream_bytes", "chfsi_bfp_encode", "chfsi_bfp_decode", "chfsi_bfp_gather_encode",
     "chfsi_bfp_decode_scatter_add",
-    "chfsi_rr_project", "chfsi_rr_rotate_workspace_bytes", "chfsi_rr_rotate", "chfsi_measure_pipe_peaks",
+    "chfsi_rr_project", "chfsi_rr_rotate_workspace_bytes", "chfsi_rr_rotate", "chfsi_rr_rotate_static", "chfsi_measure_pipe_peaks",
     "chfsi_poisson_set_quadrature", "chfsi_poisson_kdiag", "chfsi_poisson_apply_K", "chfsi_poisson_workspace_bytes", "chfsi_poisson_pcg",
     "chfsi_last_launch_count", "chfsi_last_error", "chfsi_version",
 ]
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
     L.chfsi_rr_project.argtypes = [vp, C.c_longlong, C.c_int, vp, C.c_longlong, vp, C.c_longlong, C.c_int, C.c_int, vp, vp]
     L.chfsi_rr_rotate_workspace_bytes.argtypes = [C.c_int, C.POINTER(C.c_size_t)]
     L.chfsi_rr_rotate.argtypes = [C.c_int, C.c_longlong, C.c_int, vp, C.c_longlong, vp, vp, C.c_longlong, vp, C.c_size_t, vp]
+    L.chfsi_rr_rotate_static.argtypes = [C.c_int, C.c_longlong, C.c_int, vp, C.c_longlong, vp, vp, C.c_longlong, vp]
     L.chfsi_measure_pipe_peaks.argtypes = [C.c_int, dp]
     L.chfsi_poisson_set_quadrature.argtypes = [vp, C.c_int]
     L.chfsi_poisson_kdiag.argtypes = [vp, dp]
@@ -266,6 +267,17 @@ def chfsi_rr_rotate(prec, Y, Q, Yout, work, stream=None):
     nrows = Y.numel() // Y.shape[-1]
     _check(lib().chfsi_rr_rotate(int(prec), nrows, nvec, _ptr(Y), Y.stride(-2), _ptr(Q), _ptr(Yout), Yout.stride(-2), _ptr(work),
                                  work.numel(), _stream(stream)))
+
+
+RR_STATIC_MAX_NVEC = 512
+
+
+def chfsi_rr_rotate_static(prec, Y, Q, Yout, stream=None):
+    """chfsi_rr_rotate on the library's static device scratch (no workspace, no allocation; nvec <= RR_STATIC_MAX_NVEC)."""
+    nvec = Q.shape[0]
+    nrows = Y.numel() // Y.shape[-1]
+    _check(lib().chfsi_rr_rotate_static(int(prec), nrows, nvec, _ptr(Y), Y.stride(-2), _ptr(Q), _ptr(Yout), Yout.stride(-2),
+                                        _stream(stream)))
 
 
 def chfsi_measure_pipe_peaks(device=0) -> dict:

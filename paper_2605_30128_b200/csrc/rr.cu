@@ -5,6 +5,8 @@
 // DFMA pipe (measured: DMMA 63.8, DFMA 58.5 FMA/clk/SM, the two add up when mixed -- DESIGN.md 6.6), so the projection is
 // bound by the same pipe either way; the FP32 rotation runs on FFMA so that it really is "FP32 arithmetic".
 #include <cstdint>
+#include <mutex>
+#include <string>
 
 #include "chfsi_internal.h"
 
@@ -283,3 +285,47 @@ chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const v
 }
 
 }  // extern "C"
+
+// ---- chfsi_rr_rotate_static: the rotation for callers that cannot allocate (CUDA graph capture, serving loops) ---------
+// The split-Q scratch of chfsi_rr_rotate (dq + Q with a zero diagonal) lives in this file-scope device array instead of a
+// caller buffer: kRrStaticBytes = chfsi_rr_rotate_workspace_bytes(CHFSI_RR_STATIC_MAX_NVEC) = 4,203,008 bytes, held by every
+// GPU that loads the library until the process exits.  In host code the array's NAME is a host-side stand-in, not a device
+// address; the device address is resolved once per device with cudaGetSymbolAddress (that device current) and cached.
+constexpr size_t kRrStaticBytes = (size_t)CHFSI_RR_STATIC_MAX_NVEC * CHFSI_RR_STATIC_MAX_NVEC * 16 + (size_t)CHFSI_RR_STATIC_MAX_NVEC * 16 + 512;
+static __device__ __align__(256) unsigned char g_rr_static_scratch[kRrStaticBytes];
+
+constexpr int kRrMaxDevices = 64;
+static std::mutex g_rr_static_mu;
+static void* g_rr_static_ptr[kRrMaxDevices] = {};
+
+// device address of g_rr_static_scratch on the current device (resolved on the first call per device)
+static chfsi_status rr_static_scratch(void** out) {
+    int dev = -1;
+    chfsi_status rc = rr_cuda(cudaGetDevice(&dev), "rr_rotate_static: cudaGetDevice");
+    if (rc != CHFSI_OK) return rc;
+    if (dev < 0 || dev >= kRrMaxDevices) return rr_fail(CHFSI_EUNSUPPORTED, "rr_rotate_static: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lk(g_rr_static_mu);
+    if (g_rr_static_ptr[dev] == nullptr) {
+        void* p = nullptr;
+        rc = rr_cuda(cudaGetSymbolAddress(&p, g_rr_static_scratch), "rr_rotate_static: cudaGetSymbolAddress");
+        if (rc != CHFSI_OK) return rc;
+        if (p == nullptr || ((uintptr_t)p & 255)) return rr_fail(CHFSI_ECUDA, "rr_rotate_static: scratch symbol has no 256-byte aligned device address");
+        g_rr_static_ptr[dev] = p;
+    }
+    *out = g_rr_static_ptr[dev];
+    return CHFSI_OK;
+}
+
+extern "C" chfsi_status chfsi_rr_rotate_static(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q,
+                                               void* Yout, long long ldo, void* cuda_stream) {
+    if (nvec > CHFSI_RR_STATIC_MAX_NVEC)
+        return rr_fail(CHFSI_EINVAL, "rr_rotate_static: nvec exceeds CHFSI_RR_STATIC_MAX_NVEC (512), the size of the library's static "
+                                     "scratch; use chfsi_rr_rotate with a caller workspace");
+    void* work = nullptr;
+    const chfsi_status rc = rr_static_scratch(&work);
+    if (rc != CHFSI_OK) return rc;
+    // Nothing in the scratch has to start at zero: rr_split_q_kernel overwrites dq[0, nvec) and all nvec^2 entries of Qo
+    // (zero diagonal included) before rr_rotate_kernel reads them, on the same stream; the last call's contents beyond
+    // that range are never read.  chfsi_rr_rotate itself allocates nothing (two kernel launches on `cuda_stream`).
+    return chfsi_rr_rotate(prec, nrows, nvec, Y, ldy, Q, Yout, ldo, work, kRrStaticBytes, cuda_stream);
+}
