@@ -477,8 +477,14 @@ cell_xyz_kernel(const __grid_constant__ XyzConst<typename ModeT<MODE>::TC> sc, c
 
     // ================================ consumers ================================
     // warp w: half jh = w % 2 of the rows, indices q = (w / 2) * RPW + lane / C (the half-empty warps of C = 16 come last)
-    const int q = (warp >> 1) * Cfg::RPW + lane / C;
-    if ((warp & 1) == 0) {
+    // Role r of warp w (half jh = r % 2, index group r / 2).  Warps go to the four schedulers of the SM by w % 4 and the
+    // half-0 warps carry one row more (NJ = 5 against 4 at p = 8), so the plain r = w would put every heavy warp on
+    // schedulers 0 and 2.  Ten consumer warps (p = 8, C = 16; schedulers hold 3, 3, 2 + producer, 2 warps): heavy warps on the
+    // two-warp schedulers.  Otherwise: swap the halves in every other group of four warps.
+    int role = warp ^ ((warp >> 2) & 1);
+    if (Cfg::NCW == 10) role = (int)((0x9562734081ull >> (4 * warp)) & 15);   // w: 0 1 2 3 4 5 6 7 8 9 -> r: 1 8 0 4 3 7 2 6 5 9
+    const int q = (role >> 1) * Cfg::RPW + lane / C;
+    if ((role & 1) == 0) {
         XyzConsumer<P, CC, MODE, HASPH, MASSIN, 0> cs;
         cs.init(sc, ar, q, lane % C, ex, ey, chunk, g0, xwrap, ywrap);
         cs.run(sc, ar, smem, XR, full_bar, empty_bar, T);
