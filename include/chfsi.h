@@ -205,9 +205,12 @@ chfsi_status chfsi_bfp_decode_scatter_add(int nbits, const void* src_stream, con
  *   mirrored (the caller asserts that the exact S is Hermitian); the diagonal is returned exactly real.  FP64.
  * chfsi_rr_rotate (RR-SR): Yout = Y Q.  prec CHFSI_FP32: the paper's mixed precision, "Y Q_non-diag is evaluated in FP32
  *   arithmetic, while Y Q_diag is computed in FP64" (Y and the off-diagonal of Q are rounded to complex64, products and
- *   accumulation in FP32, the result widened and added to Y Q_diag).  prec CHFSI_FP64: all FP64.  Q: device, nvec x nvec
- *   complex128, row-major.  Y and Yout must be distinct.  work: device scratch of chfsi_rr_rotate_workspace_bytes(nvec),
- *   256-byte aligned.  Diagonalising the projected pencil (RR-diag, ELPA in the paper) is left to the caller.
+ *   accumulation in FP32, the result widened and added to Y Q_diag).  prec CHFSI_FP64: all FP64.  prec CHFSI_TF32X3: the
+ *   same mixed form with the off-diagonal product on the tcgen05 tensor cores: both operands rounded to FP32 and split into
+ *   two TF32 parts, three TF32 products per term, FP32 accumulation in tensor memory (FP32-level accuracy; DESIGN.md reading
+ *   R2).  Q: device, nvec x nvec complex128, row-major.  Y and Yout must be distinct.  work: device scratch of
+ *   chfsi_rr_rotate_workspace_bytes(nvec) (enough for every precision), 256-byte aligned.  Diagonalising the projected
+ *   pencil (RR-diag, ELPA in the paper) is left to the caller.
  * EINVAL: bad sizes / leading dimensions / alignment / NULL; EUNSUPPORTED: other precisions. */
 chfsi_status chfsi_rr_project(const chfsi_mesh* mesh, long long nrows, int nvec, const void* A, long long lda,
                               const void* B, long long ldb, int use_mass, int hermitian, void* S, void* cuda_stream);
@@ -215,10 +218,10 @@ chfsi_status chfsi_rr_rotate_workspace_bytes(int nvec, size_t* bytes);
 chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q,
                              void* Yout, long long ldo, void* work, size_t work_bytes, void* cuda_stream);
 
-/* chfsi_rr_rotate_static: chfsi_rr_rotate (same operation, same arguments, layout and errors) for callers that
- * cannot allocate device memory and have no workspace to pass: code under CUDA graph capture, tight serving loops, harnesses
+/* chfsi_rr_rotate_static: chfsi_rr_rotate (same operation, same arguments, layout and errors; prec CHFSI_FP64
+ * or CHFSI_FP32 only, CHFSI_EUNSUPPORTED otherwise) for callers that cannot allocate device memory and have no workspace to pass: code under CUDA graph capture, tight serving loops, harnesses
  * that forbid cudaMalloc.  The split-Q scratch is a static device array inside the library, 4,203,008 bytes
- * (= chfsi_rr_rotate_workspace_bytes(CHFSI_RR_STATIC_MAX_NVEC)), resident on every GPU that loads the library until the
+ * (what those two precisions need at CHFSI_RR_STATIC_MAX_NVEC), resident on every GPU that loads the library until the
  * process exits.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine): it launches the same
  * two kernels as chfsi_rr_rotate on `cuda_stream`.  nvec > CHFSI_RR_STATIC_MAX_NVEC: CHFSI_EINVAL (use chfsi_rr_rotate).
  * The device address of the array is resolved on the first call on each device (cudaGetSymbolAddress with that device

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libchfsi.so")
-SOURCES = ["chfsi.cu", "kernels.cu", "cell_march.cu", "cell_xyz.cu", "cell_mma.cu", "bfp.cu", "rr.cu", "poisson.cu", "poisson_gl.cu", "peaks.cu"]
+SOURCES = ["chfsi.cu", "kernels.cu", "cell_march.cu", "cell_xyz.cu", "cell_mma.cu", "bfp.cu", "rr.cu", "rr_tc.cu", "poisson.cu", "poisson_gl.cu", "peaks.cu"]
 HEADERS = [os.path.join(CSRC, "chfsi_internal.h"), os.path.join(CSRC, "tma_util.cuh"), os.path.join(ROOT, "include", "chfsi.h")]
 
 

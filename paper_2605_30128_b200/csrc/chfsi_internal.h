@@ -184,6 +184,10 @@ bool march_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
 cudaError_t launch_cell_march(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
 // line-owned x/y/z TMA kernel (cell_xyz.cu)
 bool xyz_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);
+// Rayleigh-Ritz rotation on tcgen05 (rr_tc.cu): FP64 diagonal + 3xTF32 off-diagonal; work as laid out by rr_tc_workspace_bytes
+size_t rr_tc_workspace_bytes(int nvec);
+cudaError_t launch_rr_rotate_tc(long long nrows, int nvec, const void* Y, long long ldy, const void* Q, void* Yout, long long ldo,
+                                void* work, cudaStream_t st);
 cudaError_t launch_cell_xyz(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a, cudaStream_t s);
 // tensor-core cell kernel (cell_mma.cu): mma.sync TF32 / 3xTF32 on complex64 storage, mma.sync FP64 on complex128 storage
 bool mma_supported(const chfsi_mesh* m, chfsi_prec prec, const CellArgs& a);

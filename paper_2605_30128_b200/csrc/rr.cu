@@ -237,21 +237,27 @@ chfsi_status chfsi_rr_project(const chfsi_mesh* mesh, long long nrows, int nvec,
 chfsi_status chfsi_rr_rotate_workspace_bytes(int nvec, size_t* bytes) {
     if (!bytes || nvec < 1) return rr_fail(CHFSI_EINVAL, "rr_rotate_workspace_bytes: bad argument");
     *bytes = (size_t)nvec * nvec * 16 + (size_t)nvec * 16 + 512;
+    if (rr_tc_workspace_bytes(nvec) > *bytes) *bytes = rr_tc_workspace_bytes(nvec);   // CHFSI_TF32X3 (rr_tc.cu)
     return CHFSI_OK;
 }
 
 chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q, void* Yout,
                              long long ldo, void* work, size_t work_bytes, void* cuda_stream) {
-    if (prec != CHFSI_FP64 && prec != CHFSI_FP32) return rr_fail(CHFSI_EUNSUPPORTED, "rr_rotate: prec must be CHFSI_FP64 or CHFSI_FP32 (mixed, PAPER.md:232)");
+    if (prec != CHFSI_FP64 && prec != CHFSI_FP32 && prec != CHFSI_TF32X3)
+        return rr_fail(CHFSI_EUNSUPPORTED, "rr_rotate: prec must be CHFSI_FP64, CHFSI_FP32 (mixed, PAPER.md:232) or CHFSI_TF32X3 (mixed on tcgen05)");
     if (nvec < 1 || nrows < 0) return rr_fail(CHFSI_EINVAL, "rr_rotate: nvec must be >= 1 and nrows >= 0");
     if (!Y || !Q || !Yout || !work) return rr_fail(CHFSI_EINVAL, "rr_rotate: NULL device pointer");
     if (Y == Yout) return rr_fail(CHFSI_EINVAL, "rr_rotate: Y and Yout must be distinct buffers");
     if (ldy < nvec || ldo < nvec) return rr_fail(CHFSI_EINVAL, "rr_rotate: leading dimension < nvec");
-    size_t need = 0;
-    chfsi_rr_rotate_workspace_bytes(nvec, &need);
+    // what this precision needs (chfsi_rr_rotate_workspace_bytes returns the largest over the precisions)
+    const size_t need = prec == CHFSI_TF32X3 ? rr_tc_workspace_bytes(nvec) : (size_t)nvec * nvec * 16 + (size_t)nvec * 16 + 512;
     if (work_bytes < need || ((uintptr_t)work & 255)) return rr_fail(CHFSI_EINVAL, "rr_rotate: work too small or not 256-byte aligned");
     if (((uintptr_t)Y & 15) || ((uintptr_t)Q & 15) || ((uintptr_t)Yout & 15)) return rr_fail(CHFSI_EINVAL, "rr_rotate: pointers must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (prec == CHFSI_TF32X3) {
+        if (nrows >= (1ll << 31) * 128) return rr_fail(CHFSI_EINVAL, "rr_rotate: too many rows");
+        return rr_cuda(launch_rr_rotate_tc(nrows, nvec, Y, ldy, Q, Yout, ldo, work, st), "rr_rotate (tcgen05)");
+    }
     double2* dq = static_cast<double2*>(work);
     void* qo = static_cast<char*>(work) + (((size_t)nvec * 16 + 255) / 256) * 256;
     const long long n2 = (long long)nvec * nvec;
@@ -288,7 +294,7 @@ chfsi_status chfsi_rr_rotate(chfsi_prec prec, long long nrows, int nvec, const v
 
 // ---- chfsi_rr_rotate_static: the rotation for callers that cannot allocate (CUDA graph capture, serving loops) ---------
 // The split-Q scratch of chfsi_rr_rotate (dq + Q with a zero diagonal) lives in this file-scope device array instead of a
-// caller buffer: kRrStaticBytes = chfsi_rr_rotate_workspace_bytes(CHFSI_RR_STATIC_MAX_NVEC) = 4,203,008 bytes, held by every
+// caller buffer: kRrStaticBytes = what the FP64 and FP32 paths need at CHFSI_RR_STATIC_MAX_NVEC = 4,203,008 bytes, held by every
 // GPU that loads the library until the process exits.  In host code the array's NAME is a host-side stand-in, not a device
 // address; the device address is resolved once per device with cudaGetSymbolAddress (that device current) and cached.
 constexpr size_t kRrStaticBytes = (size_t)CHFSI_RR_STATIC_MAX_NVEC * CHFSI_RR_STATIC_MAX_NVEC * 16 + (size_t)CHFSI_RR_STATIC_MAX_NVEC * 16 + 512;
@@ -318,6 +324,8 @@ static chfsi_status rr_static_scratch(void** out) {
 
 extern "C" chfsi_status chfsi_rr_rotate_static(chfsi_prec prec, long long nrows, int nvec, const void* Y, long long ldy, const void* Q,
                                                void* Yout, long long ldo, void* cuda_stream) {
+    if (prec != CHFSI_FP64 && prec != CHFSI_FP32)
+        return rr_fail(CHFSI_EUNSUPPORTED, "rr_rotate_static: prec must be CHFSI_FP64 or CHFSI_FP32 (the static scratch holds the split Q of those two paths only)");
     if (nvec > CHFSI_RR_STATIC_MAX_NVEC)
         return rr_fail(CHFSI_EINVAL, "rr_rotate_static: nvec exceeds CHFSI_RR_STATIC_MAX_NVEC (512), the size of the library's static "
                                      "scratch; use chfsi_rr_rotate with a caller workspace");

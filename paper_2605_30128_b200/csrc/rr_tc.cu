@@ -1,0 +1,266 @@
+// Rayleigh-Ritz subspace rotation on the 5th-generation tensor cores (tcgen05 + TMEM), sm_100a only.
+//
+//   Yout = Y Q_diag (FP64)  +  Y Q_non-diag (3xTF32 on tcgen05.mma.kind::tf32, FP32 accumulation in TMEM)
+//
+// PAPER.md:232 evaluates Y Q_non-diag "in FP32 arithmetic" and Y Q_diag in FP64.  Here the off-diagonal product runs as
+// three TF32 tensor-core products per term (x = hi + lo, hi = tf32(x), lo = tf32(x - hi); lo*hi + hi*lo + hi*hi, FP32
+// accumulation): 21 operand bits, FP32-level accuracy (reading R2), at the tensor pipe's rate instead of FFMA's.
+//
+// Real form of the complex product.  A row of Y is 2 nvec reals (re, im interleaved) = the K index k' = 2 i + c; an output
+// row is 2 nvec reals, column j' = 2 j + d.  B[k'][j'] = Qre_ij (c == d), Qim_ij (c = 0, d = 1), -Qim_ij (c = 1, d = 0).
+//
+// One CTA = 128 rows x 256 real output columns (M = 128, N = 256: one accumulator of 256 TMEM columns), K in chunks of 32
+// reals (128-byte rows, the 128-byte swizzle of the UMMA shared-memory layout).  Warp roles:
+//   warps 0-3 : converters -- load the FP64 rows of Y, round to FP32, split into hi / lo, store the two A tiles in the
+//               swizzled K-major layout (generic proxy -> fence.proxy.async -> mbarrier); afterwards the epilogue: TMEM ->
+//               registers (tcgen05.ld 32x32b), + Y Q_diag in FP64, store complex128.
+//   warp 4    : one lane streams the pre-split, pre-swizzled B tiles (hi, lo; 32 KB each, contiguous in the workspace) with
+//               cp.async.bulk onto an mbarrier.
+//   warp 5    : allocates TMEM; one lane issues the tcgen05.mma's (12 per chunk) and commits them to the stage's `empty`
+//               barrier and, after the last chunk, to `acc_full`.
+// Two shared-memory stages of 96 KB (A hi/lo 2 x 16 KB, B hi/lo 2 x 32 KB).
+#include <algorithm>
+#include <cstdint>
+#include <mutex>
+#include <string>
+
+#include "chfsi_internal.h"
+#include "tma_util.cuh"
+
+namespace chfsi {
+
+constexpr int TC_M = 128, TC_N = 256, TC_KC = 32, TC_STAGES = 2;
+constexpr int TC_A_BYTES = TC_M * 128, TC_B_BYTES = TC_N * 128;
+constexpr int TC_STAGE_BYTES = 2 * TC_A_BYTES + 2 * TC_B_BYTES;
+constexpr int TC_SMEM = TC_STAGES * TC_STAGE_BYTES + 1024;      // + slack to align the tiles to 1024 bytes
+constexpr int TC_THREADS = 192;
+
+__device__ __forceinline__ float tf32_rna(float x) {
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return __uint_as_float(r);
+}
+
+// UMMA shared-memory descriptor of a K-major tile with 128-byte rows and the 128-byte swizzle: 8-row groups are 1024 bytes
+// apart (SBO), the leading-dimension offset is unused for swizzled K-major operands, version 1 (sm_100), layout type 2.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)1 << 16;
+    d |= (uint64_t)(1024 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+
+// instruction descriptor: D = F32 (bits 4-5 = 1), A = B = TF32 (bits 7-9, 10-12 = 2), both K-major, N / 8 at bit 17, M / 16 at bit 24
+constexpr uint32_t TC_IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
+
+__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(TC_IDESC), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// ---- Q -> dq (FP64 diagonal) and the real-form off-diagonal B, split into TF32 hi / lo, in the layout the kernel's stages
+//      hold: tile (nh, kc) = 256 rows (n) x 32 reals (k), 128-byte rows, 16-byte chunks XOR-swizzled by n % 8.
+__global__ void rr_tc_split_q_kernel(const double2* __restrict__ Q, int nvec, int kchunks, int nhalves, double2* __restrict__ dq,
+                                     float* __restrict__ Bhi, float* __restrict__ Blo) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)nhalves * kchunks * TC_N * TC_KC;
+    if (idx < nvec) dq[idx] = Q[idx * nvec + idx];
+    if (idx >= total) return;
+    const int k = (int)(idx % TC_KC);
+    const int n = (int)((idx / TC_KC) % TC_N);
+    const long long tile = idx / (TC_KC * TC_N);
+    const int kc = (int)(tile % kchunks), nh = (int)(tile / kchunks);
+    const int kp = kc * TC_KC + k, jp = nh * TC_N + n;
+    const int i = kp >> 1, c = kp & 1, j = jp >> 1, d = jp & 1;
+    double v = 0.0;
+    if (i < nvec && j < nvec && i != j) {
+        const double2 q = Q[(long long)i * nvec + j];
+        v = (c == d) ? q.x : (c == 0 ? q.y : -q.y);
+    }
+    const float xf = (float)v;
+    const float hi = tf32_rna(xf), lo = tf32_rna(xf - hi);
+    const long long off = (tile * TC_N + n) * TC_KC + ((((k >> 2) ^ (n & 7)) << 2) | (k & 3));
+    Bhi[off] = hi;
+    Blo[off] = lo;
+}
+
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+          "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+          "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+__global__ void __launch_bounds__(TC_THREADS, 1)
+rr_rotate_tc_kernel(const double2* __restrict__ Y, long long ldy, const float* __restrict__ Bhi, const float* __restrict__ Blo,
+                    const double2* __restrict__ dq, long long nrows, int nvec, int kchunks, double2* __restrict__ C, long long ldc) {
+    extern __shared__ unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t a_full[TC_STAGES], b_full[TC_STAGES], empty[TC_STAGES], acc_full;
+    __shared__ uint32_t tmem_base_s;
+    unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // tiles on 1024-byte boundaries
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long m0 = (long long)blockIdx.x * TC_M;
+    const int nh = blockIdx.y;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&a_full[s], 128); mbar_init(&b_full[s], 1); mbar_init(&empty[s], 1); }
+        mbar_init(&acc_full, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 5) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(2 * TC_N) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = tmem_base_s;
+
+    if (warp < 4) {
+        // ============ converters: FP64 rows of Y -> FP32 -> TF32 hi / lo, swizzled K-major A tiles ============
+        const int cpx = threadIdx.x & 15;                  // complex column within the chunk (16 per chunk of 32 reals)
+        const int rsub = threadIdx.x >> 4;                 // 8 rows per pass
+        double2 y[16], yn[16];
+        auto load_chunk = [&](int c, double2 (&dst)[16]) {
+            const int i = c * (TC_KC / 2) + cpx;
+#pragma unroll
+            for (int pass = 0; pass < 16; ++pass) {
+                const long long r = m0 + pass * 8 + rsub;
+                dst[pass] = make_double2(0.0, 0.0);
+                if (c < kchunks && r < nrows && i < nvec) dst[pass] = __ldg(Y + r * ldy + i);
+            }
+        };
+        load_chunk(0, y);
+        for (int c = 0; c < kchunks; ++c) {
+            const int s = c & 1;
+            load_chunk(c + 1, yn);                           // the next chunk's loads are in flight while this one is converted
+            if (c >= TC_STAGES) mbar_wait(&empty[s], ((c >> 1) - 1) & 1);
+            unsigned char* Ahi = smem + (size_t)s * TC_STAGE_BYTES;
+            unsigned char* Alo = Ahi + TC_A_BYTES;
+#pragma unroll
+            for (int pass = 0; pass < 16; ++pass) {
+                const int row = pass * 8 + rsub;
+                const float xr = (float)y[pass].x, xi = (float)y[pass].y;
+                const float hr = tf32_rna(xr), hi_ = tf32_rna(xi);
+                const float lr = tf32_rna(xr - hr), li = tf32_rna(xi - hi_);
+                const uint32_t off = (uint32_t)row * 128u + ((uint32_t)((cpx >> 1) ^ (row & 7)) << 4) + (uint32_t)(cpx & 1) * 8u;
+                *reinterpret_cast<float2*>(Ahi + off) = make_float2(hr, hi_);
+                *reinterpret_cast<float2*>(Alo + off) = make_float2(lr, li);
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> visible to the tensor core
+            mbar_arrive(&a_full[s]);
+#pragma unroll
+            for (int pass = 0; pass < 16; ++pass) y[pass] = yn[pass];
+        }
+        // ============ epilogue: TMEM -> registers, + Y Q_diag (FP64), store ============
+        mbar_wait(&acc_full, 0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const long long r = m0 + warp * 32 + lane;          // TMEM lane = row of the tile; warp w reads lanes 32 w ...
+        const uint32_t tlane = tmem + ((uint32_t)(warp * 32) << 16);
+#pragma unroll 1
+        for (int cb = 0; cb < TC_N / 32; ++cb) {
+            uint32_t v[32], w[32];
+            tmem_ld32(tlane + (uint32_t)(cb * 32), v);
+            tmem_ld32(tlane + (uint32_t)(TC_N + cb * 32), w);
+            const int j0 = nh * (TC_N / 2) + cb * 16;
+            if (r < nrows) {
+#pragma unroll
+                for (int jj = 0; jj < 16; ++jj) {
+                    const int j = j0 + jj;
+                    if (j < nvec) {
+                        const double2 yv = __ldg(Y + r * ldy + j), d = dq[j];      // Y Q_diag in FP64
+                        C[r * ldc + j] = make_double2(fma(yv.x, d.x, fma(-yv.y, d.y, (double)(__uint_as_float(v[2 * jj]) + __uint_as_float(w[2 * jj])))),
+                                                      fma(yv.x, d.y, fma(yv.y, d.x, (double)(__uint_as_float(v[2 * jj + 1]) + __uint_as_float(w[2 * jj + 1])))));
+                    }
+                }
+            }
+        }
+    } else if (warp == 4) {
+        // ============ B loader ============
+        if (lane == 0) {
+            for (int c = 0; c < kchunks; ++c) {
+                const int s = c & 1;
+                if (c >= TC_STAGES) mbar_wait(&empty[s], ((c >> 1) - 1) & 1);
+                unsigned char* Bh = smem + (size_t)s * TC_STAGE_BYTES + 2 * TC_A_BYTES;
+                const size_t off = ((size_t)nh * kchunks + c) * (TC_N * TC_KC);
+                mbar_expect_tx(&b_full[s], 2 * TC_B_BYTES);
+                bulk_load(Bh, Bhi + off, TC_B_BYTES, &b_full[s]);
+                bulk_load(Bh + TC_B_BYTES, Blo + off, TC_B_BYTES, &b_full[s]);
+            }
+        }
+    } else {
+        // ============ MMA issuer ============
+        if (lane == 0) {
+            for (int c = 0; c < kchunks; ++c) {
+                const int s = c & 1;
+                mbar_wait(&a_full[s], (c >> 1) & 1);
+                mbar_wait(&b_full[s], (c >> 1) & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t a_hi = smem_u32(smem + (size_t)s * TC_STAGE_BYTES), a_lo = a_hi + TC_A_BYTES;
+                const uint32_t b_hi = a_hi + 2 * TC_A_BYTES, b_lo = b_hi + TC_B_BYTES;
+#pragma unroll
+                for (int ks = 0; ks < TC_KC / 8; ++ks) {               // K = 8 TF32 (32 bytes) per instruction
+                    const uint64_t dah = umma_desc_sw128(a_hi + ks * 32), dal = umma_desc_sw128(a_lo + ks * 32);
+                    const uint64_t dbh = umma_desc_sw128(b_hi + ks * 32), dbl = umma_desc_sw128(b_lo + ks * 32);
+                    // two accumulators: the tensor core truncates when it adds into FP32, once per instruction, so the error grows
+                    // with the number of instructions that hit an accumulator; the cross terms (small) get their own
+                    umma_tf32(tmem + TC_N, dal, dbh, (c | ks) != 0 ? 1u : 0u);
+                    umma_tf32(tmem + TC_N, dah, dbl, 1u);
+                    umma_tf32(tmem, dah, dbh, (c | ks) != 0 ? 1u : 0u);
+                }
+                umma_commit(&empty[s]);                                  // frees the stage when these MMAs have read it
+            }
+            umma_commit(&acc_full);
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 5) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(2 * TC_N) : "memory");
+}
+
+// workspace: dq (nvec complex128, padded to 256 bytes) | B hi | B lo
+size_t rr_tc_workspace_bytes(int nvec) {
+    const size_t kchunks = (2 * (size_t)nvec + TC_KC - 1) / TC_KC, nhalves = (2 * (size_t)nvec + TC_N - 1) / TC_N;
+    return (((size_t)nvec * 16 + 255) / 256) * 256 + 2 * nhalves * kchunks * TC_N * TC_KC * sizeof(float) + 256;
+}
+
+cudaError_t launch_rr_rotate_tc(long long nrows, int nvec, const void* Y, long long ldy, const void* Q, void* Yout, long long ldo,
+                                void* work, cudaStream_t st) {
+    const int kchunks = (2 * nvec + TC_KC - 1) / TC_KC, nhalves = (2 * nvec + TC_N - 1) / TC_N;
+    double2* dq = static_cast<double2*>(work);
+    float* Bhi = reinterpret_cast<float*>(static_cast<char*>(work) + (((size_t)nvec * 16 + 255) / 256) * 256);
+    float* Blo = Bhi + (size_t)nhalves * kchunks * TC_N * TC_KC;
+    const long long total = std::max<long long>((long long)nhalves * kchunks * TC_N * TC_KC, nvec);
+    rr_tc_split_q_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(static_cast<const double2*>(Q), nvec, kchunks, nhalves, dq, Bhi, Blo);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    count_launch();
+    if (nrows == 0) return cudaSuccess;
+    static std::once_flag once[32];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaError_t ae = cudaSuccess;
+    std::call_once(once[dev & 31], [&] { ae = cudaFuncSetAttribute(rr_rotate_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM); });
+    if (ae != cudaSuccess) return ae;
+    const dim3 grid((unsigned)((nrows + TC_M - 1) / TC_M), (unsigned)nhalves);
+    rr_rotate_tc_kernel<<<grid, TC_THREADS, TC_SMEM, st>>>(static_cast<const double2*>(Y), ldy, Bhi, Blo, dq, nrows, nvec, kchunks,
+                                                           static_cast<double2*>(Yout), ldo);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) count_launch();
+    return e;
+}
+
+}  // namespace chfsi

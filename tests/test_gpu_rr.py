@@ -3,7 +3,9 @@
 Tolerances: the projection is FP64 with a different summation order than the oracle's matmul (split rows, REDs): relative
 Frobenius 1e-12.  The mixed-precision rotation is FP32 in its off-diagonal part on both sides, in different summation orders:
 relative Frobenius 1e-5 (north_star's FP32-inexact bar) and, as a property, within the FP32 bound of the exact FP64 product;
-the FP64 rotation: 1e-13."""
+the FP64 rotation: 1e-13.  The tcgen05 rotation (CHFSI_TF32X3: FP64 diagonal + 3xTF32 off-diagonal, FP32 accumulation in tensor
+memory) is held to the same two bars as the FP32 one (measured 1e-7 ... 1.3e-6 on these cases).  Several row tiles, both column
+halves, ragged K chunks and ragged rows are covered by the sizes below and by test_rotate_tcgen05_tiles."""
 import numpy as np
 import pytest
 
@@ -69,7 +71,7 @@ def test_project_with_mass_on_a_mesh_and_rr_eigenvalues(env, ro):
         Q = Li.conj().T @ Z
         Qd = torch.from_numpy(Q).cuda()
         work = torch.empty(B.chfsi_rr_rotate_workspace_bytes(24), dtype=torch.uint8, device="cuda")
-        for prec, mixed, tol in [(B.FP64, False, 1e-13), (B.FP32, True, 1e-5)]:
+        for prec, mixed, tol in [(B.FP64, False, 1e-13), (B.FP32, True, 1e-5), (B.TF32X3, True, 1e-5)]:
             Xd = torch.full_like(Yd, float("nan"))
             B.chfsi_rr_rotate(prec, Yd, Qd, Xd, work)
             X = Xd.cpu().numpy().reshape(-1, 24)
@@ -93,7 +95,7 @@ def test_rotate_fp64_and_mixed(env, ro, nrows, nvec, ld):
     for Q in (U, near, np.eye(nvec, dtype=np.complex128)):
         Qd = torch.from_numpy(np.ascontiguousarray(Q)).cuda()
         exact = ro.rr_rotate(Y[:, :nvec], Q, mixed=False)
-        for prec, mixed, tol in [(B.FP64, False, 1e-13), (B.FP32, True, 1e-5)]:
+        for prec, mixed, tol in [(B.FP64, False, 1e-13), (B.FP32, True, 1e-5), (B.TF32X3, True, 1e-5)]:
             out = torch.full((nrows, ld), float("nan"), dtype=torch.complex128, device="cuda")
             B.chfsi_rr_rotate(prec, Yd[:, :nvec], Qd, out[:, :nvec], work)
             got = out.cpu().numpy()[:, :nvec]
@@ -106,6 +108,24 @@ def test_rotate_fp64_and_mixed(env, ro, nrows, nvec, ld):
         B.chfsi_rr_rotate(B.FP64, Yd[:, :nvec], Qd, Yd[:, :nvec], work)                      # in place is refused
     with pytest.raises(B.ChfsiError):
         B.chfsi_rr_rotate(B.TF32, Yd[:, :nvec], Qd, out[:, :nvec], work)
+
+
+@pytest.mark.parametrize("nrows,nvec", [(1, 1), (127, 15), (129, 16), (1000, 128), (385, 129), (2500, 300)])
+def test_rotate_tcgen05_tiles(env, ro, nrows, nvec):
+    """The tcgen05 rotation across its tile boundaries: 1 / 2 / 3 column tiles of 128 vectors, ragged 16-vector K chunks, ragged
+    128-row tiles; against the oracle's mixed product and the exact FP64 one, elementwise as well as in norm."""
+    torch, _, B = env
+    rng = np.random.default_rng(1000 * nvec + nrows)
+    Y = _rand(rng, nrows, nvec)
+    Q = _rand(rng, nvec, nvec) / np.sqrt(nvec)
+    work = torch.empty(B.chfsi_rr_rotate_workspace_bytes(nvec), dtype=torch.uint8, device="cuda")
+    out = torch.full((nrows, nvec), float("nan"), dtype=torch.complex128, device="cuda")
+    B.chfsi_rr_rotate(B.TF32X3, torch.from_numpy(Y).cuda(), torch.from_numpy(Q).cuda(), out, work)
+    got = out.cpu().numpy()
+    exact = Y @ Q
+    assert np.isfinite(got).all()
+    assert relerr(got, ro.rr_rotate(Y, Q, True)) < 1e-5 and relerr(got, exact) < 1e-5
+    assert np.abs(got - exact).max() < 1e-4 * np.abs(exact).max()
 
 
 def test_project_full_size_block_properties(env, ro):
