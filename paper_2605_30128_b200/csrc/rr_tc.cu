@@ -33,7 +33,9 @@ constexpr int TC_M = 128, TC_N = 256, TC_KC = 32, TC_STAGES = 2;
 constexpr int TC_A_BYTES = TC_M * 128, TC_B_BYTES = TC_N * 128;
 constexpr int TC_STAGE_BYTES = 2 * TC_A_BYTES + 2 * TC_B_BYTES;
 constexpr int TC_SMEM = TC_STAGES * TC_STAGE_BYTES + 1024;      // + slack to align the tiles to 1024 bytes
-constexpr int TC_THREADS = 192;
+constexpr int TC_CONV_WARPS = 8, TC_CONV_THREADS = 32 * TC_CONV_WARPS;        // converters; then 4 epilogue warps, loader, MMA
+constexpr int TC_LOAD_WARP = TC_CONV_WARPS + 4, TC_MMA_WARP = TC_CONV_WARPS + 5;
+constexpr int TC_THREADS = 32 * (TC_CONV_WARPS + 6);
 
 __device__ __forceinline__ float tf32_rna(float x) {
     uint32_t r;
@@ -104,23 +106,28 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
+// Persistent: grid = number of SMs; a CTA walks tiles blockIdx.x, blockIdx.x + gridDim.x, ... (tile = 128 rows x one column
+// half; the halves of a row tile are consecutive tile numbers, so they run at the same time on neighbouring SMs and the
+// second read of the rows hits L2).  Chunks are numbered g = 0, 1, ... across the tiles of the CTA; stage g % 2.
 __global__ void __launch_bounds__(TC_THREADS, 1)
 rr_rotate_tc_kernel(const double2* __restrict__ Y, long long ldy, const float* __restrict__ Bhi, const float* __restrict__ Blo,
-                    const double2* __restrict__ dq, long long nrows, int nvec, int kchunks, double2* __restrict__ C, long long ldc) {
+                    const double2* __restrict__ dq, long long nrows, int nvec, int kchunks, int nhalves, long long ntiles,
+                    double2* __restrict__ C, long long ldc) {
     extern __shared__ unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t a_full[TC_STAGES], b_full[TC_STAGES], empty[TC_STAGES], acc_full;
+    __shared__ __align__(8) uint64_t a_full[TC_STAGES], b_full[TC_STAGES], empty[TC_STAGES], acc_full, acc_empty;
     __shared__ uint32_t tmem_base_s;
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // tiles on 1024-byte boundaries
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long m0 = (long long)blockIdx.x * TC_M;
-    const int nh = blockIdx.y;
+    const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const long long nchunks_total = my_tiles * kchunks;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&a_full[s], 128); mbar_init(&b_full[s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&a_full[s], TC_CONV_THREADS); mbar_init(&b_full[s], 1); mbar_init(&empty[s], 1); }
         mbar_init(&acc_full, 1);
+        mbar_init(&acc_empty, 128);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 5) {
+    if (warp == TC_MMA_WARP) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(2 * TC_N) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -129,31 +136,39 @@ rr_rotate_tc_kernel(const double2* __restrict__ Y, long long ldy, const float* _
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = tmem_base_s;
 
-    if (warp < 4) {
+    if (warp < TC_CONV_WARPS) {
         // ============ converters: FP64 rows of Y -> FP32 -> TF32 hi / lo, swizzled K-major A tiles ============
-        const int cpx = threadIdx.x & 15;                  // complex column within the chunk (16 per chunk of 32 reals)
-        const int rsub = threadIdx.x >> 4;                 // 8 rows per pass
-        double2 y[16], yn[16];
-        auto load_chunk = [&](int c, double2 (&dst)[16]) {
+        // 256 threads: 16 threads per row (one complex each), 16 rows per pass, 8 passes per chunk; the loads of the next two
+        // chunks are in flight while a chunk is converted (64 KB per SM)
+        constexpr int NP = TC_M / (TC_CONV_THREADS / 16);
+        const int cpx = threadIdx.x & 15;
+        const int rsub = threadIdx.x >> 4;
+        double2 y0[NP], y1[NP], y2[NP];
+        auto load_chunk = [&](long long g, double2 (&dst)[NP]) {
+            const long long ti = g / kchunks;
+            const int c = (int)(g - ti * kchunks);
+            const long long tile = blockIdx.x + ti * gridDim.x;
+            const long long m0 = (tile / nhalves) * TC_M;
             const int i = c * (TC_KC / 2) + cpx;
 #pragma unroll
-            for (int pass = 0; pass < 16; ++pass) {
-                const long long r = m0 + pass * 8 + rsub;
+            for (int pass = 0; pass < NP; ++pass) {
+                const long long r = m0 + pass * (TC_M / NP) + rsub;
                 dst[pass] = make_double2(0.0, 0.0);
-                if (c < kchunks && r < nrows && i < nvec) dst[pass] = __ldg(Y + r * ldy + i);
+                if (g < nchunks_total && r < nrows && i < nvec) dst[pass] = __ldg(Y + r * ldy + i);
             }
         };
-        load_chunk(0, y);
-        for (int c = 0; c < kchunks; ++c) {
-            const int s = c & 1;
-            load_chunk(c + 1, yn);                           // the next chunk's loads are in flight while this one is converted
-            if (c >= TC_STAGES) mbar_wait(&empty[s], ((c >> 1) - 1) & 1);
+        load_chunk(0, y0);
+        load_chunk(1, y1);
+        for (long long g = 0; g < nchunks_total; ++g) {
+            const int s = (int)(g & 1);
+            load_chunk(g + 2, y2);
+            if (g >= TC_STAGES) mbar_wait(&empty[s], (uint32_t)(((g >> 1) - 1) & 1));
             unsigned char* Ahi = smem + (size_t)s * TC_STAGE_BYTES;
             unsigned char* Alo = Ahi + TC_A_BYTES;
 #pragma unroll
-            for (int pass = 0; pass < 16; ++pass) {
-                const int row = pass * 8 + rsub;
-                const float xr = (float)y[pass].x, xi = (float)y[pass].y;
+            for (int pass = 0; pass < NP; ++pass) {
+                const int row = pass * (TC_M / NP) + rsub;
+                const float xr = (float)y0[pass].x, xi = (float)y0[pass].y;
                 const float hr = tf32_rna(xr), hi_ = tf32_rna(xi);
                 const float lr = tf32_rna(xr - hr), li = tf32_rna(xi - hi_);
                 const uint32_t off = (uint32_t)row * 128u + ((uint32_t)((cpx >> 1) ^ (row & 7)) << 4) + (uint32_t)(cpx & 1) * 8u;
@@ -163,37 +178,51 @@ rr_rotate_tc_kernel(const double2* __restrict__ Y, long long ldy, const float* _
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> visible to the tensor core
             mbar_arrive(&a_full[s]);
 #pragma unroll
-            for (int pass = 0; pass < 16; ++pass) y[pass] = yn[pass];
+            for (int pass = 0; pass < NP; ++pass) { y0[pass] = y1[pass]; y1[pass] = y2[pass]; }
         }
+    } else if (warp < TC_CONV_WARPS + 4) {
         // ============ epilogue: TMEM -> registers, + Y Q_diag (FP64), store ============
-        mbar_wait(&acc_full, 0);
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const long long r = m0 + warp * 32 + lane;          // TMEM lane = row of the tile; warp w reads lanes 32 w ...
-        const uint32_t tlane = tmem + ((uint32_t)(warp * 32) << 16);
+        const int ew = warp - TC_CONV_WARPS;                 // = warp % 4: this warp reads TMEM lanes 32 ew ... 32 ew + 31
+        const uint32_t tlane = tmem + ((uint32_t)(ew * 32) << 16);
+        for (long long ti = 0; ti < my_tiles; ++ti) {
+            const long long tile = blockIdx.x + ti * gridDim.x;
+            const long long r = (tile / nhalves) * TC_M + ew * 32 + lane;
+            const int nh = (int)(tile % nhalves);
+            mbar_wait(&acc_full, (uint32_t)(ti & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
-        for (int cb = 0; cb < TC_N / 32; ++cb) {
-            uint32_t v[32], w[32];
-            tmem_ld32(tlane + (uint32_t)(cb * 32), v);
-            tmem_ld32(tlane + (uint32_t)(TC_N + cb * 32), w);
-            const int j0 = nh * (TC_N / 2) + cb * 16;
-            if (r < nrows) {
+            for (int cb = 0; cb < TC_N / 32; ++cb) {
+                uint32_t v[32], w[32];
+                tmem_ld32(tlane + (uint32_t)(cb * 32), v);
+                tmem_ld32(tlane + (uint32_t)(TC_N + cb * 32), w);
+                if (cb == TC_N / 32 - 1) {                   // the accumulators are in registers: the next tile may overwrite them
+                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                    mbar_arrive(&acc_empty);
+                }
+                const int j0 = nh * (TC_N / 2) + cb * 16;
+                if (r < nrows) {
 #pragma unroll
-                for (int jj = 0; jj < 16; ++jj) {
-                    const int j = j0 + jj;
-                    if (j < nvec) {
-                        const double2 yv = __ldg(Y + r * ldy + j), d = dq[j];      // Y Q_diag in FP64
-                        C[r * ldc + j] = make_double2(fma(yv.x, d.x, fma(-yv.y, d.y, (double)(__uint_as_float(v[2 * jj]) + __uint_as_float(w[2 * jj])))),
-                                                      fma(yv.x, d.y, fma(yv.y, d.x, (double)(__uint_as_float(v[2 * jj + 1]) + __uint_as_float(w[2 * jj + 1])))));
+                    for (int jj = 0; jj < 16; ++jj) {
+                        const int j = j0 + jj;
+                        if (j < nvec) {
+                            const double2 yv = __ldg(Y + r * ldy + j), d = dq[j];      // Y Q_diag in FP64
+                            C[r * ldc + j] = make_double2(
+                                fma(yv.x, d.x, fma(-yv.y, d.y, (double)(__uint_as_float(v[2 * jj]) + __uint_as_float(w[2 * jj])))),
+                                fma(yv.x, d.y, fma(yv.y, d.x, (double)(__uint_as_float(v[2 * jj + 1]) + __uint_as_float(w[2 * jj + 1])))));
+                        }
                     }
                 }
             }
         }
-    } else if (warp == 4) {
+    } else if (warp == TC_LOAD_WARP) {
         // ============ B loader ============
         if (lane == 0) {
-            for (int c = 0; c < kchunks; ++c) {
-                const int s = c & 1;
-                if (c >= TC_STAGES) mbar_wait(&empty[s], ((c >> 1) - 1) & 1);
+            for (long long g = 0; g < nchunks_total; ++g) {
+                const int s = (int)(g & 1);
+                const long long ti = g / kchunks;
+                const int c = (int)(g - ti * kchunks);
+                const int nh = (int)((blockIdx.x + ti * gridDim.x) % nhalves);
+                if (g >= TC_STAGES) mbar_wait(&empty[s], (uint32_t)(((g >> 1) - 1) & 1));
                 unsigned char* Bh = smem + (size_t)s * TC_STAGE_BYTES + 2 * TC_A_BYTES;
                 const size_t off = ((size_t)nh * kchunks + c) * (TC_N * TC_KC);
                 mbar_expect_tx(&b_full[s], 2 * TC_B_BYTES);
@@ -204,31 +233,38 @@ rr_rotate_tc_kernel(const double2* __restrict__ Y, long long ldy, const float* _
     } else {
         // ============ MMA issuer ============
         if (lane == 0) {
-            for (int c = 0; c < kchunks; ++c) {
-                const int s = c & 1;
-                mbar_wait(&a_full[s], (c >> 1) & 1);
-                mbar_wait(&b_full[s], (c >> 1) & 1);
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t a_hi = smem_u32(smem + (size_t)s * TC_STAGE_BYTES), a_lo = a_hi + TC_A_BYTES;
-                const uint32_t b_hi = a_hi + 2 * TC_A_BYTES, b_lo = b_hi + TC_B_BYTES;
-#pragma unroll
-                for (int ks = 0; ks < TC_KC / 8; ++ks) {               // K = 8 TF32 (32 bytes) per instruction
-                    const uint64_t dah = umma_desc_sw128(a_hi + ks * 32), dal = umma_desc_sw128(a_lo + ks * 32);
-                    const uint64_t dbh = umma_desc_sw128(b_hi + ks * 32), dbl = umma_desc_sw128(b_lo + ks * 32);
-                    // two accumulators: the tensor core truncates when it adds into FP32, once per instruction, so the error grows
-                    // with the number of instructions that hit an accumulator; the cross terms (small) get their own
-                    umma_tf32(tmem + TC_N, dal, dbh, (c | ks) != 0 ? 1u : 0u);
-                    umma_tf32(tmem + TC_N, dah, dbl, 1u);
-                    umma_tf32(tmem, dah, dbh, (c | ks) != 0 ? 1u : 0u);
+            long long g = 0;
+            for (long long ti = 0; ti < my_tiles; ++ti) {
+                if (ti > 0) {                                               // the epilogue has read the previous tile's accumulators
+                    mbar_wait(&acc_empty, (uint32_t)((ti - 1) & 1));
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 }
-                umma_commit(&empty[s]);                                  // frees the stage when these MMAs have read it
+                for (int c = 0; c < kchunks; ++c, ++g) {
+                    const int s = (int)(g & 1);
+                    mbar_wait(&a_full[s], (uint32_t)((g >> 1) & 1));
+                    mbar_wait(&b_full[s], (uint32_t)((g >> 1) & 1));
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t a_hi = smem_u32(smem + (size_t)s * TC_STAGE_BYTES), a_lo = a_hi + TC_A_BYTES;
+                    const uint32_t b_hi = a_hi + 2 * TC_A_BYTES, b_lo = b_hi + TC_B_BYTES;
+#pragma unroll
+                    for (int ks = 0; ks < TC_KC / 8; ++ks) {               // K = 8 TF32 (32 bytes) per instruction
+                        const uint64_t dah = umma_desc_sw128(a_hi + ks * 32), dal = umma_desc_sw128(a_lo + ks * 32);
+                        const uint64_t dbh = umma_desc_sw128(b_hi + ks * 32), dbl = umma_desc_sw128(b_lo + ks * 32);
+                        // two accumulators: the tensor core truncates when it adds into FP32, once per instruction, so the error
+                        // grows with the number of instructions that hit an accumulator; the (small) cross terms get their own
+                        umma_tf32(tmem + TC_N, dal, dbh, (c | ks) != 0 ? 1u : 0u);
+                        umma_tf32(tmem + TC_N, dah, dbl, 1u);
+                        umma_tf32(tmem, dah, dbh, (c | ks) != 0 ? 1u : 0u);
+                    }
+                    umma_commit(&empty[s]);                                  // frees the stage when these MMAs have read it
+                }
+                umma_commit(&acc_full);
             }
-            umma_commit(&acc_full);
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 5) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(2 * TC_N) : "memory");
+    if (warp == TC_MMA_WARP) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(2 * TC_N) : "memory");
 }
 
 // workspace: dq (nvec complex128, padded to 256 bytes) | B hi | B lo
@@ -255,9 +291,12 @@ cudaError_t launch_rr_rotate_tc(long long nrows, int nvec, const void* Y, long l
     cudaError_t ae = cudaSuccess;
     std::call_once(once[dev & 31], [&] { ae = cudaFuncSetAttribute(rr_rotate_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM); });
     if (ae != cudaSuccess) return ae;
-    const dim3 grid((unsigned)((nrows + TC_M - 1) / TC_M), (unsigned)nhalves);
+    int nsm = 0;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    const long long ntiles = ((nrows + TC_M - 1) / TC_M) * nhalves;
+    const unsigned grid = (unsigned)std::min<long long>(ntiles, nsm > 0 ? nsm : 148);
     rr_rotate_tc_kernel<<<grid, TC_THREADS, TC_SMEM, st>>>(static_cast<const double2*>(Y), ldy, Bhi, Blo, dq, nrows, nvec, kchunks,
-                                                           static_cast<double2*>(Yout), ldo);
+                                                           nhalves, ntiles, static_cast<double2*>(Yout), ldo);
     e = cudaGetLastError();
     if (e == cudaSuccess) count_launch();
     return e;
