@@ -399,6 +399,15 @@ def all_configs_table(torch, B, device, peak):
 
 
 
+def tf32_tensor_peak():
+    """Dense TF32 tensor peak in TFLOP/s: the measured bf16 peak x the nominal ratio of B200_PROFILING.md (1.1 / 2.25 PFLOP/s)."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["bf16_tflops"]) * 1.1 / 2.25, "MEASURED_PEAKS.json bf16_tflops x 1.1 / 2.25 (nominal TF32 : bf16)"
+    except Exception:
+        return 1100.0, "nominal 1.1 PFLOP/s dense TF32 (B200_PROFILING.md; MEASURED_PEAKS.json absent)"
+
+
 def extra_kernels(torch, B, device, hbm_peak, pipe):
     """Rows for the NEXT components that are not part of a filter step: the BFP codec (HBM-bound) and the Rayleigh-Ritz
     projection / rotation (FMA-pipe bound; the roof is the issue rate measured in this run by chfsi_measure_pipe_peaks)."""
@@ -460,6 +469,15 @@ def extra_kernels(torch, B, device, hbm_peak, pipe):
             rows.append({"kernel": nm, "rows": nrows, "nvec": nv, "ms": round(t, 3), "bound": "alu",
                          "achieved_TFs": round(flops / (t * 1e-3) / 1e12, 2), "peak_TFs": round(pipe[pk], 2),
                          "frac": round(flops / (t * 1e-3) / 1e12 / pipe[pk], 4), "dtype": "f32 off-diagonal / f64 diagonal" if prec == B.FP32 else "f64"})
+        # the same mixed rotation on tcgen05 (3xTF32): three TF32 products per term are executed; roof = the TF32 tensor peak,
+        # taken as the measured bf16 peak of MEASURED_PEAKS.json x the guide's nominal TF32 : bf16 ratio (1.1 : 2.25)
+        t = timed(lambda: B.chfsi_rr_rotate(B.TF32X3, Y, Q, Yo, wk), reps=3)
+        tf32_peak, tf32_src = tf32_tensor_peak()
+        rows.append({"kernel": "rr_rotate (FP64 diagonal + 3xTF32 off-diagonal on tcgen05)", "rows": nrows, "nvec": nv, "ms": round(t, 3),
+                     "bound": "tensor", "achieved_TFs": round(3 * flops / (t * 1e-3) / 1e12, 2), "peak_TFs": round(tf32_peak, 1),
+                     "frac": round(3 * flops / (t * 1e-3) / 1e12 / tf32_peak, 4), "peak_source": tf32_src,
+                     "useful_TFs": round(flops / (t * 1e-3) / 1e12, 2), "hbm_GBs": round(2.0 * nrows * nv * 16 / (t * 1e-3) / 1e9, 1),
+                     "dtype": "tf32 x3 off-diagonal (f32 accumulation) / f64 diagonal"})
     finally:
         B.chfsi_mesh_destroy(mesh)
         torch.cuda.empty_cache()

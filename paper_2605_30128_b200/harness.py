@@ -103,8 +103,8 @@ class GpuProblem:
 
     def rayleigh_ritz(self, Y, lib_rr=None):
         """Alg. 1 lines 6-9: Y^H H Y Q = Y^H M Y Q Lambda; returns (Y Q, Lambda).  lib_rr = None: projection and rotation
-        with torch dense algebra; lib_rr = B.FP64 / B.FP32: with the library's chfsi_rr_project and chfsi_rr_rotate (FP32 =
-        the paper's FP64-diagonal + FP32-off-diagonal rotation).  The small dense eigenproblem stays in torch."""
+        with torch dense algebra; lib_rr = B.FP64 / B.FP32 / B.TF32X3: with the library's chfsi_rr_project and chfsi_rr_rotate (FP32 =
+        the paper's FP64-diagonal + FP32-off-diagonal rotation; TF32X3 = the same on tcgen05, 3xTF32 off-diagonal).  The small dense eigenproblem stays in torch."""
         t = self.torch
         M2 = 2 * self.nnodes
         nv = Y.shape[-1]

@@ -161,7 +161,7 @@ def test_eigenvalues_fp32_filter_vs_dense_oracle(env):
         # every inexact mode, incl. single-pass TF32 (its per-call error is 1e-3: what it is held to is this), and
         # the library's own Rayleigh-Ritz kernels with the paper's mixed-precision rotation
         for prec, lib_rr in ((B.FP32, None), (B.FP64, None), (B.FP32_STORED, None), (B.TF32X3, None), (B.TF32, None),
-                             (B.FP64, B.FP64), (B.TF32, B.FP32)):
+                             (B.FP64, B.FP64), (B.TF32, B.FP32), (B.FP32_STORED, B.TF32X3)):   # TF32X3 rotation = tcgen05 (rr_tc.cu)
             lam, hist = _converge(pb, X0, cfg.degree, b, prec, 1e-6, n_check, 200, lib_rr=lib_rr)
             assert hist[-1] <= 1e-6, (prec, lib_rr, hist[-5:])
             err = np.max(np.abs(lam[:n_check] - exact[:n_check]))
