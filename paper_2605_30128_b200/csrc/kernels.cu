@@ -211,6 +211,11 @@ template <typename TS> struct C2Sel;
 template <> struct C2Sel<double> { using type = double2; };
 template <> struct C2Sel<float> { using type = float2; };
 __device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
+// one complex value per reduction: a single red.global.add.v2.f32 for complex64 (8-byte aligned), two RED.ADD.F64 for complex128
+__device__ __forceinline__ void red_add2(float* p, float re, float im) {
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(re), "f"(im) : "memory");
+}
+__device__ __forceinline__ void red_add2(double* p, double re, double im) { atomicAdd(p, re); atomicAdd(p + 1, im); }
 
 // TT: arithmetic type of the contraction; TS: storage type of the multivectors (double: complex128, float: complex64)
 template <typename TT, typename TS>
@@ -436,8 +441,7 @@ back_fast_kernel(const NonlocalDev nl, const BackArgs ar) {
             yi = fma(pv.x, g_i[b], fma(pv.y, g_r[b], yi));
         }
         TS* dst = out + 4 * nodes[jj] * ar.ld_out;
-        red_add(dst, (TS)(fac[jj] * (double)yr));
-        red_add(dst + 1, (TS)(fac[jj] * (double)yi));
+        red_add2(dst, (TS)(fac[jj] * (double)yr), (TS)(fac[jj] * (double)yi));
     }
 }
 
