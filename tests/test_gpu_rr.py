@@ -110,9 +110,9 @@ def test_rotate_fp64_and_mixed(env, ro, nrows, nvec, ld):
         B.chfsi_rr_rotate(B.TF32, Yd[:, :nvec], Qd, out[:, :nvec], work)
 
 
-@pytest.mark.parametrize("nrows,nvec", [(1, 1), (127, 15), (129, 16), (1000, 128), (385, 129), (2500, 300)])
+@pytest.mark.parametrize("nrows,nvec", [(1, 1), (127, 15), (129, 16), (1000, 128), (385, 129), (2500, 300), (200, 1024)])
 def test_rotate_tcgen05_tiles(env, ro, nrows, nvec):
-    """The tcgen05 rotation across its tile boundaries: 1 / 2 / 3 column tiles of 128 vectors, ragged 16-vector K chunks, ragged
+    """The tcgen05 rotation across its tile boundaries: 1 / 2 / 3 / 8 column tiles of 128 vectors, ragged 16-vector K chunks, ragged
     128-row tiles; against the oracle's mixed product and the exact FP64 one, elementwise as well as in norm."""
     torch, _, B = env
     rng = np.random.default_rng(1000 * nvec + nrows)
