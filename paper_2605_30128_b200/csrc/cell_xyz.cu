@@ -162,7 +162,7 @@ struct XyzConsumer {
         own_a = a < P;
         WXa = sc.WX[a]; WYa = sc.WY[a]; mxa = sc.M1X[a];
 #pragma unroll
-        for (int l = 0; l < NJ; ++l) wxy[l] = WXa * sc.WY[RS::row(l)];
+        for (int l = 0; l < NJ; ++l) wxy[l] = MODE == M_F64 ? (TC)0 : WXa * sc.WY[RS::row(l)];
         cin = (vok && ar.cin) ? __ldg(ar.cin + v) : 0.0;
         cR = (vok && ar.cR && ar.useR) ? __ldg(ar.cR + v) : 0.0;
         rowoff = a * P * C + col; faceoff = (n * P + a) * C + col;            // X-phase: row q of the plane
@@ -304,7 +304,12 @@ struct XyzConsumer {
         }
         TC zr[NJ];
 #pragma unroll
-        for (int l = 0; l < NJ; ++l) zr[l] = wxy[l] * v[RS::row(l)];
+        for (int l = 0; l < NJ; ++l) {
+            // FP64: the product W_x[a] W_y[row] is not kept per thread (NJ double registers under the 168-register cap); the
+            // weight of the row comes from the constant bank and the association keeps the compiler from hoisting it back
+            if constexpr (MODE == M_F64) zr[l] = WXa * (sc.WY[RS::row(l)] * v[RS::row(l)]);
+            else zr[l] = wxy[l] * v[RS::row(l)];
+        }
         if (lower) {
 #pragma unroll
             for (int k = 0; k < n; ++k) {
