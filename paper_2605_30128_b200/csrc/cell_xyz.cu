@@ -222,7 +222,10 @@ struct XyzConsumer {
     __device__ __forceinline__ void add_plane(TC wzc, const TC (&ip)[NJ], const TC (&s5)[NJ]) {
         if constexpr (K < n) {
 #pragma unroll
-            for (int l = 0; l < NJ; ++l) acc[K][l] += fma(wzc, ip[l], s5[l]);
+            for (int l = 0; l < NJ; ++l) {
+                if constexpr (MODE == M_F64) acc[K][l] += ip[l];          // ip already holds w_z ip + S5
+                else acc[K][l] += fma(wzc, ip[l], s5[l]);
+            }
         }
     }
 
@@ -336,9 +339,17 @@ struct XyzConsumer {
 #pragma unroll
                 for (int l = 0; l < NJ; ++l) acc[k][l] = fma(kz, zr[l], acc[k][l]);
             }
+            // FP64: S5 is folded into the in-plane part as it is formed (ip <- w_z ip + S5), so no second array of NJ values is live
+            const TC wzc = sc.WZ[c];
             TC s5[NJ];
 #pragma unroll
             for (int l = 0; l < NJ; ++l) s5[l] = (TC)0;
+            if constexpr (MODE == M_F64) {
+                if (!own_a) {
+#pragma unroll
+                    for (int l = 0; l < NJ; ++l) ip[l] = wzc * ip[l];
+                }
+            }
             if (own_a) {
                 // S5 on the owned nodes of this plane (rows < P at x-position a < P): eq. 12 spin blocks, in-term, R-term
                 const int nb = a * C + col;
@@ -372,11 +383,13 @@ struct XyzConsumer {
                         if (MASSIN) val *= mzx * sc.M1Y[j];              // the residual S0: H X - M X Lambda carries m_I
                         if (ar.useR) val = fma(cR, Rs[o], val);
                         if (MODE == M_F32P) { if (emit_ok) red_add(p5 + (long long)j * LS, (TO)val); }
+                        else if (MODE == M_F64) ip[l] = fma(wzc, ip[l], (TC)val);
                         else s5[l] = (TC)val;
+                    } else if (MODE == M_F64) {
+                        ip[l] = wzc * ip[l];
                     }
                 }
             }
-            const TC wzc = sc.WZ[c];
             switch (c) {
                 case 0: add_plane<0>(wzc, ip, s5); break;
                 case 1: add_plane<(1 < P ? 1 : n)>(wzc, ip, s5); break;
