@@ -116,6 +116,7 @@ rr_rotate_tc_kernel(const double2* __restrict__ Y, long long ldy, const float* _
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t a_full[TC_STAGES], b_full[TC_STAGES], empty[TC_STAGES], acc_full, acc_empty;
     __shared__ uint32_t tmem_base_s;
+    __shared__ float stash[4 * 32 * 33];                     // epilogue transpose, one 32 x 32 block (+ padding) per epilogue warp
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // tiles on 1024-byte boundaries
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
@@ -186,30 +187,49 @@ rr_rotate_tc_kernel(const double2* __restrict__ Y, long long ldy, const float* _
         const uint32_t tlane = tmem + ((uint32_t)(ew * 32) << 16);
         for (long long ti = 0; ti < my_tiles; ++ti) {
             const long long tile = blockIdx.x + ti * gridDim.x;
-            const long long r = (tile / nhalves) * TC_M + ew * 32 + lane;
             const int nh = (int)(tile % nhalves);
             mbar_wait(&acc_full, (uint32_t)(ti & 1));
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            // tcgen05.ld hands a thread one ROW (32 columns of it).  Loads and stores of 32 rows x 16 bytes per instruction cost 32
+            // LSU wavefronts each (measured: LSU data pipe 67 % busy, the epilogue's 16.7 us of wavefronts per tile were the kernel's
+            // bottleneck), so the block is transposed through shared memory: afterwards a half-warp covers the 16 complex values
+            // (256 bytes) of one row, for the loads of Y (diagonal term) and the stores alike -- 4 wavefronts per instruction.
+            float* st = stash + ew * (32 * 33);
+            const long long rbase = (tile / nhalves) * TC_M + ew * 32;
 #pragma unroll 1
             for (int cb = 0; cb < TC_N / 32; ++cb) {
-                uint32_t v[32], w[32];
-                tmem_ld32(tlane + (uint32_t)(cb * 32), v);
-                tmem_ld32(tlane + (uint32_t)(TC_N + cb * 32), w);
-                if (cb == TC_N / 32 - 1) {                   // the accumulators are in registers: the next tile may overwrite them
-                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                    mbar_arrive(&acc_empty);
-                }
-                const int j0 = nh * (TC_N / 2) + cb * 16;
-                if (r < nrows) {
+                const int j = nh * (TC_N / 2) + cb * 16 + (lane & 15);
+                const bool jok = j < nvec;
+                // the 16 values of Y this lane needs for the block (rows 2 it + lane / 16), all in flight before the TMEM reads
+                double2 yv[16];
 #pragma unroll
-                    for (int jj = 0; jj < 16; ++jj) {
-                        const int j = j0 + jj;
-                        if (j < nvec) {
-                            const double2 yv = __ldg(Y + r * ldy + j), d = dq[j];      // Y Q_diag in FP64
-                            C[r * ldc + j] = make_double2(
-                                fma(yv.x, d.x, fma(-yv.y, d.y, (double)(__uint_as_float(v[2 * jj]) + __uint_as_float(w[2 * jj])))),
-                                fma(yv.x, d.y, fma(yv.y, d.x, (double)(__uint_as_float(v[2 * jj + 1]) + __uint_as_float(w[2 * jj + 1])))));
-                        }
+                for (int it = 0; it < 16; ++it) {
+                    const long long r = rbase + it * 2 + (lane >> 4);
+                    yv[it] = make_double2(0.0, 0.0);
+                    if (r < nrows && jok) yv[it] = __ldg(Y + r * ldy + j);
+                }
+                const double2 d = jok ? dq[j] : make_double2(0.0, 0.0);
+                {
+                    uint32_t v[32], w[32];
+                    tmem_ld32(tlane + (uint32_t)(cb * 32), v);
+                    tmem_ld32(tlane + (uint32_t)(TC_N + cb * 32), w);
+                    if (cb == TC_N / 32 - 1) {               // the accumulators are in registers: the next tile may overwrite them
+                        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                        mbar_arrive(&acc_empty);
+                    }
+                    __syncwarp();                            // the previous block's reads of the stash are done
+#pragma unroll
+                    for (int q = 0; q < 32; ++q) st[lane * 33 + q] = __uint_as_float(v[q]) + __uint_as_float(w[q]);
+                }
+                __syncwarp();
+#pragma unroll
+                for (int it = 0; it < 16; ++it) {
+                    const int rr = it * 2 + (lane >> 4);
+                    const long long r = rbase + rr;
+                    if (r < nrows && jok) {
+                        const float are = st[rr * 33 + 2 * (lane & 15)], aim = st[rr * 33 + 2 * (lane & 15) + 1];
+                        C[r * ldc + j] = make_double2(fma(yv[it].x, d.x, fma(-yv[it].y, d.y, (double)are)),      // Y Q_diag in FP64
+                                                      fma(yv[it].x, d.y, fma(yv[it].y, d.x, (double)aim)));
                     }
                 }
             }
