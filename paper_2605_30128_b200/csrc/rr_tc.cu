@@ -170,8 +170,12 @@ rr_rotate_tc_kernel(const double2* __restrict__ Y, long long ldy, const float* _
             for (int pass = 0; pass < NP; ++pass) {
                 const int row = pass * (TC_M / NP) + rsub;
                 const float xr = (float)y0[pass].x, xi = (float)y0[pass].y;
-                const float hr = tf32_rna(xr), hi_ = tf32_rna(xi);
-                const float lr = tf32_rna(xr - hr), li = tf32_rna(xi - hi_);
+                // hi = x rounded to TF32, nearest-away, with two integer operations (half a TF32 ulp added to the magnitude bits, the low
+                // 13 bits cleared: what cvt.rna.tf32.f32 returns for finite x, without its conversion-pipe slot); lo = x - hi is exact in
+                // FP32 and goes to the tensor core as it is, which reads its upper 19 bits
+                const float hr = __uint_as_float((__float_as_uint(xr) + 0x1000u) & 0xFFFFE000u);
+                const float hi_ = __uint_as_float((__float_as_uint(xi) + 0x1000u) & 0xFFFFE000u);
+                const float lr = xr - hr, li = xi - hi_;
                 const uint32_t off = (uint32_t)row * 128u + ((uint32_t)((cpx >> 1) ^ (row & 7)) << 4) + (uint32_t)(cpx & 1) * 8u;
                 *reinterpret_cast<float2*>(Ahi + off) = make_float2(hr, hi_);
                 *reinterpret_cast<float2*>(Alo + off) = make_float2(lr, li);
